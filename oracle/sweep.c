@@ -1,0 +1,304 @@
+/* ORACLE — test infrastructure, not product code.
+ *
+ * Plain fp64 CPU implementation of the DOCTORS hot path, written from the paper
+ * and the readings in DESIGN.md / SURVEY.md §8(c).  It shares no
+ * code with the CUDA library.  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs may call it.
+ *
+ * What is here (each function cites the passage it follows):
+ *   orc_wavefront_size   P(S), Eqs. (9)-(22)
+ *   orc_schedule         sub-sweep membership and order, PAPER.md:72-81 (Eq. 8), Table 1 (:121-139)
+ *   orc_sweep            one transport sweep of Eq. (2) over all directions,
+ *                        diamond difference, vacuum boundaries (:37),
+ *                        scalar flux / moments by Eq. (3) (:39)
+ *   orc_raytrace         uncollided fluence of Eq. (4) by exact voxel ray tracing
+ *
+ * Layouts: cell c = i + nx*(j + ny*k) (x fastest); moments [nm][cells]; all double.
+ * Threads (OpenMP) split independent directions / rays only; every sum that
+ * crosses threads is done in a fixed order, so results do not depend on the
+ * thread count.
+ */
+#define _USE_MATH_DEFINES
+#define _GNU_SOURCE
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+/* ---- PAPER.md:85-117, Eqs. (9)-(22): number of voxels in sub-sweep S ---- */
+static int64_t tri(int64_t d) { return d * (d + 1) / 2; }
+static int64_t pos(int64_t v) { return v > 0 ? v : 0; }
+
+int64_t orc_wavefront_size(int nx, int ny, int nz, int S)
+{
+    int64_t Cs  = (int64_t)(S + 1) * (S + 2) / 2;              /* Eq. (10) */
+    int64_t dx  = pos((int64_t)S + 1 - nx);                    /* Eq. (17) */
+    int64_t dy  = pos((int64_t)S + 1 - ny);                    /* Eq. (18), "d_v" read as d_y */
+    int64_t dz  = pos((int64_t)S + 1 - nz);                    /* Eq. (19) */
+    int64_t dxy = pos((int64_t)S + 1 - nx - ny);               /* Eq. (20) */
+    int64_t dyz = pos((int64_t)S + 1 - ny - nz);               /* Eq. (21) */
+    int64_t dxz = pos((int64_t)S + 1 - nx - nz);               /* Eq. (22) */
+    return Cs - tri(dx) - tri(dy) - tri(dz) + tri(dxy) + tri(dyz) + tri(dxz);   /* Eq. (9), (11)-(16) */
+}
+
+/* ---- PAPER.md:72-81 Eq. (8) + Table 1: cells of every sub-sweep, in Table 1 order ----
+ * Sweep-space indices (i',j',k') with i'+j'+k' = S, 0 <= i' < nx etc.  Table 1 lists
+ * i' descending, then j' descending.  Octant bit0/1/2 set = sweep runs in -x/-y/-z,
+ * so the mesh index is mirrored: i = nx-1-i'.
+ * plane_offset has nx+ny+nz-1 entries, cell_of has nx*ny*nz. */
+void orc_schedule(int nx, int ny, int nz, int octant, int32_t *plane_offset, int32_t *cell_of)
+{
+    int planes = nx + ny + nz - 2;
+    int64_t n = 0;
+    for (int S = 0; S < planes; ++S) {
+        plane_offset[S] = (int32_t)n;
+        for (int ip = (S < nx - 1 ? S : nx - 1); ip >= 0; --ip) {
+            for (int jp = (S - ip < ny - 1 ? S - ip : ny - 1); jp >= 0; --jp) {
+                int kp = S - ip - jp;
+                if (kp >= nz) break;                 /* smaller j' only makes k' larger */
+                int i = (octant & 1) ? nx - 1 - ip : ip;
+                int j = (octant & 2) ? ny - 1 - jp : jp;
+                int k = (octant & 4) ? nz - 1 - kp : kp;
+                cell_of[n++] = (int32_t)(i + nx * (j + ny * k));
+            }
+        }
+    }
+    plane_offset[planes] = (int32_t)n;
+}
+
+/* ---- one cell, one direction: diamond difference (textbook DD of ref. 13) ----
+ * Balance over the cell + psi_c = (psi_in + psi_out)/2 on each axis:
+ *   psi_c = (q + cx*pin_x + cy*pin_y + cz*pin_z) / (sigt + cx + cy + cz),  c_d = 2|Omega_d|/Delta_d
+ *   pout_d = 2 psi_c - pin_d
+ * closure 1 (reading R2): any outflow < 0 is set to 0 and the balance is re-solved with that
+ * face's DD relation dropped; repeat while new faces flip (at most 3 rounds). */
+static inline double dd_cell(double q, double sigt, const double c[3], const double pin[3],
+                             int closure, double pout[3], int64_t *nfix)
+{
+    int fixed[3] = {0, 0, 0};
+    double psi = 0.0;
+    for (int pass = 0; pass < 4; ++pass) {
+        double num = q, den = sigt;
+        for (int d = 0; d < 3; ++d) {
+            if (fixed[d]) num += 0.5 * c[d] * pin[d];
+            else { num += c[d] * pin[d]; den += c[d]; }
+        }
+        psi = num / den;
+        int flipped = 0;
+        for (int d = 0; d < 3; ++d) {
+            pout[d] = fixed[d] ? 0.0 : 2.0 * psi - pin[d];
+            if (closure == 1 && !fixed[d] && pout[d] < 0.0) { fixed[d] = 1; flipped = 1; }
+        }
+        if (!flipped) break;
+        if (nfix) ++*nfix;
+    }
+    for (int d = 0; d < 3; ++d) if (fixed[d]) pout[d] = 0.0;
+    return psi;
+}
+
+/* sweep one direction in lexicographic upwind order; psi[cells] out; returns leakage
+ * sum over outflow boundary faces of |Omega_d| * A_d * psi_out  (not yet weighted by w_n). */
+static double sweep_dir_lex(int nx, int ny, int nz, const double del[3], const double *sigt,
+                            const double *qn, const double om[3], int closure,
+                            double *psi, int64_t *nfix)
+{
+    double c[3] = {2.0 * fabs(om[0]) / del[0], 2.0 * fabs(om[1]) / del[1], 2.0 * fabs(om[2]) / del[2]};
+    double area[3] = {del[1] * del[2], del[0] * del[2], del[0] * del[1]};
+    double *fy = (double *)calloc((size_t)nx, sizeof(double));
+    double *fz = (double *)calloc((size_t)nx * ny, sizeof(double));
+    double leak = 0.0;
+    for (int kp = 0; kp < nz; ++kp) {
+        int k = om[2] > 0 ? kp : nz - 1 - kp;
+        for (int ip = 0; ip < nx; ++ip) fy[ip] = 0.0;           /* vacuum inflow on the y face (:37) */
+        for (int jp = 0; jp < ny; ++jp) {
+            int j = om[1] > 0 ? jp : ny - 1 - jp;
+            double fx = 0.0;                                      /* vacuum inflow on the x face */
+            for (int ip = 0; ip < nx; ++ip) {
+                int i = om[0] > 0 ? ip : nx - 1 - ip;
+                size_t cidx = (size_t)i + (size_t)nx * (j + (size_t)ny * k);
+                double pin[3] = {fx, fy[i], kp == 0 ? 0.0 : fz[i + (size_t)nx * j]};
+                double pout[3];
+                psi[cidx] = dd_cell(qn[cidx], sigt[cidx], c, pin, closure, pout, nfix);
+                fx = pout[0]; fy[i] = pout[1]; fz[i + (size_t)nx * j] = pout[2];
+                if (ip == nx - 1) leak += fabs(om[0]) * area[0] * pout[0];
+                if (jp == ny - 1) leak += fabs(om[1]) * area[1] * pout[1];
+                if (kp == nz - 1) leak += fabs(om[2]) * area[2] * pout[2];
+            }
+        }
+    }
+    free(fy); free(fz);
+    return leak;
+}
+
+/* same direction, but cells visited in the paper's sub-sweep order (Eq. 8 / Table 1).
+ * Each cell reads its three upwind neighbours' outflows from full per-cell face arrays. */
+static double sweep_dir_hyperplane(int nx, int ny, int nz, const double del[3], const double *sigt,
+                                   const double *qn, const double om[3], int closure,
+                                   double *psi, int64_t *nfix)
+{
+    size_t cells = (size_t)nx * ny * nz;
+    int octant = (om[0] < 0 ? 1 : 0) | (om[1] < 0 ? 2 : 0) | (om[2] < 0 ? 4 : 0);
+    int planes = nx + ny + nz - 2;
+    int32_t *off = (int32_t *)malloc(sizeof(int32_t) * (planes + 1));
+    int32_t *cell_of = (int32_t *)malloc(sizeof(int32_t) * cells);
+    double *ox = (double *)malloc(sizeof(double) * cells * 3), *oy = ox + cells, *oz = oy + cells;
+    orc_schedule(nx, ny, nz, octant, off, cell_of);
+    double c[3] = {2.0 * fabs(om[0]) / del[0], 2.0 * fabs(om[1]) / del[1], 2.0 * fabs(om[2]) / del[2]};
+    double area[3] = {del[1] * del[2], del[0] * del[2], del[0] * del[1]};
+    int sx = om[0] > 0 ? 1 : -1, sy = om[1] > 0 ? 1 : -1, sz = om[2] > 0 ? 1 : -1;
+    double leak = 0.0;
+    for (int S = 0; S < planes; ++S)
+        for (int32_t t = off[S]; t < off[S + 1]; ++t) {
+            size_t cidx = (size_t)cell_of[t];
+            int i = (int)(cidx % nx), j = (int)((cidx / nx) % ny), k = (int)(cidx / ((size_t)nx * ny));
+            int iu = i - sx, ju = j - sy, ku = k - sz;               /* upwind neighbours */
+            double pin[3];
+            pin[0] = (iu < 0 || iu >= nx) ? 0.0 : ox[(size_t)iu + (size_t)nx * (j + (size_t)ny * k)];
+            pin[1] = (ju < 0 || ju >= ny) ? 0.0 : oy[(size_t)i + (size_t)nx * (ju + (size_t)ny * k)];
+            pin[2] = (ku < 0 || ku >= nz) ? 0.0 : oz[(size_t)i + (size_t)nx * (j + (size_t)ny * ku)];
+            double pout[3];
+            psi[cidx] = dd_cell(qn[cidx], sigt[cidx], c, pin, closure, pout, nfix);
+            ox[cidx] = pout[0]; oy[cidx] = pout[1]; oz[cidx] = pout[2];
+            if (i + sx < 0 || i + sx >= nx) leak += fabs(om[0]) * area[0] * pout[0];
+            if (j + sy < 0 || j + sy >= ny) leak += fabs(om[1]) * area[1] * pout[1];
+            if (k + sz < 0 || k + sz >= nz) leak += fabs(om[2]) * area[2] * pout[2];
+        }
+    free(off); free(cell_of); free(ox);
+    return leak;
+}
+
+/* ---- one sweep of Eq. (2) over all directions; moments by Eq. (3) ----
+ * Q    [nm][cells]  source moments (4pi-integrated convention, reading R6)
+ * Mtab [ndir][nm]   (2l+1)/(4pi) Y_lm(Omega_n)       -> q_n = sum_lm Mtab[n][lm] Q_lm   (Eq. 2 rhs, moment form R3)
+ * Dtab [nm][ndir]   w_n Y_lm(Omega_n)                -> phi_lm += Dtab[lm][n] psi_n     (Eq. 3)
+ * Directions are ordered octant-major (octant o = n / (ndir/8)); they are processed
+ * octant by octant, directions of the octant in index order, and summed in that order.
+ * order: 0 lexicographic loops, 1 the paper's sub-sweep order.
+ * psi_all: NULL or [ndir][cells] (angular flux, for tests).
+ * leak_out: sum_n w_n * leakage_n.   nfix_out: NULL or fix-up event count. */
+void orc_sweep(int nx, int ny, int nz, double dx, double dy, double dz,
+               const double *sigt, const double *Q, int nm,
+               int ndir, const double *omega, const double *w,
+               const double *Mtab, const double *Dtab,
+               int closure, int order,
+               double *phi, double *leak_out, double *psi_all, int64_t *nfix_out, int nthreads)
+{
+    size_t cells = (size_t)nx * ny * nz;
+    double del[3] = {dx, dy, dz};
+    int chunk = ndir / 8 > 0 && ndir % 8 == 0 ? ndir / 8 : ndir;   /* directions summed per batch */
+    double *psi_buf = (double *)malloc(sizeof(double) * cells * chunk);
+    double *qn_buf = (double *)malloc(sizeof(double) * cells * chunk);
+    double *leak_n = (double *)calloc((size_t)ndir, sizeof(double));
+    int64_t *nfix_n = (int64_t *)calloc((size_t)ndir, sizeof(int64_t));
+    memset(phi, 0, sizeof(double) * cells * nm);
+    if (nthreads < 1) nthreads = 1;
+    for (int n0 = 0; n0 < ndir; n0 += chunk) {
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads)
+        for (int m = 0; m < chunk; ++m) {
+            int n = n0 + m;
+            double *qn = qn_buf + cells * m, *psi = psi_buf + cells * m;
+            for (size_t c = 0; c < cells; ++c) {
+                double q = 0.0;
+                for (int lm = 0; lm < nm; ++lm) q += Mtab[(size_t)n * nm + lm] * Q[(size_t)lm * cells + c];
+                qn[c] = q;
+            }
+            if (order == 0) leak_n[n] = sweep_dir_lex(nx, ny, nz, del, sigt, qn, omega + 3 * n, closure, psi, nfix_n + n);
+            else leak_n[n] = sweep_dir_hyperplane(nx, ny, nz, del, sigt, qn, omega + 3 * n, closure, psi, nfix_n + n);
+            if (psi_all) memcpy(psi_all + cells * n, psi, sizeof(double) * cells);
+        }
+#pragma omp parallel for schedule(static) num_threads(nthreads)
+        for (int lm = 0; lm < nm; ++lm)
+            for (int m = 0; m < chunk; ++m) {                      /* Eq. (3): fixed direction order */
+                double d = Dtab[(size_t)lm * ndir + n0 + m];
+                const double *psi = psi_buf + cells * m;
+                double *p = phi + (size_t)lm * cells;
+                for (size_t c = 0; c < cells; ++c) p[c] += d * psi[c];
+            }
+    }
+    double leak = 0.0;
+    int64_t nf = 0;
+    for (int n = 0; n < ndir; ++n) { leak += w[n] * leak_n[n]; nf += nfix_n[n]; }
+    if (leak_out) *leak_out = leak;
+    if (nfix_out) *nfix_out = nf;
+    free(psi_buf); free(qn_buf); free(leak_n); free(nfix_n);
+}
+
+/* ---- PAPER.md:44-49 Eq. (4): uncollided fluence by ray tracing (reading R11, R12) ----
+ * For every cell centre r_c:  d = r_c - r_s, R = |d|, u = d/R.
+ *   kind 2 (cone): u . axis >= cos_half, else phi_u = 0.
+ *   The segment [0,R] is clipped to the mesh box (outside is vacuum) and walked voxel by
+ *   voxel (parametric traversal: per axis the next boundary crossing tMax and the step
+ *   tDelta; always step the axis with the smallest tMax).  Per material m the areal
+ *   density A_m = sum rho * length is accumulated (independent of the group), then
+ *     tau_g = sum_m sigt_hat[m][g] A_m,   phi_u^g = S_g exp(-tau_g) / (4 pi R^2).
+ * mesh centred on the origin.  phi_u [G][cells]; areal NULL or [n_mat][cells]. */
+void orc_raytrace(int nx, int ny, int nz, double dx, double dy, double dz,
+                  const uint8_t *mat, const double *rho, int n_mat, int G, const double *sigt_hat,
+                  int kind, const double *spos, const double *axis, double cos_half,
+                  const double *spectrum, double *phi_u, double *areal, int nthreads)
+{
+    size_t cells = (size_t)nx * ny * nz;
+    int nn[3] = {nx, ny, nz};
+    double del[3] = {dx, dy, dz};
+    double lo[3] = {-0.5 * nx * dx, -0.5 * ny * dy, -0.5 * nz * dz};
+    double an = sqrt(axis[0] * axis[0] + axis[1] * axis[1] + axis[2] * axis[2]);
+    if (nthreads < 1) nthreads = 1;
+#pragma omp parallel for schedule(static) num_threads(nthreads)
+    for (int64_t cc = 0; cc < (int64_t)cells; ++cc) {
+        size_t c = (size_t)cc;
+        int ci[3] = {(int)(c % nx), (int)((c / nx) % ny), (int)(c / ((size_t)nx * ny))};
+        double rc[3], d[3], u[3], R2 = 0.0;
+        double A[16];
+        for (int m = 0; m < n_mat; ++m) A[m] = 0.0;
+        for (int a = 0; a < 3; ++a) { rc[a] = lo[a] + (ci[a] + 0.5) * del[a]; d[a] = rc[a] - spos[a]; R2 += d[a] * d[a]; }
+        double R = sqrt(R2);
+        for (int a = 0; a < 3; ++a) u[a] = d[a] / R;
+        int lit = 1;
+        if (kind == 2) {
+            double ca = (u[0] * axis[0] + u[1] * axis[1] + u[2] * axis[2]) / an;
+            if (ca < cos_half) lit = 0;
+        }
+        if (lit) {
+            /* clip [0,R] to the box: entry parameter */
+            double t0 = 0.0;
+            for (int a = 0; a < 3; ++a) {
+                if (u[a] > 0.0) { double t = (lo[a] - spos[a]) / u[a]; if (t > t0) t0 = t; }
+                else if (u[a] < 0.0) { double t = (lo[a] + nn[a] * del[a] - spos[a]) / u[a]; if (t > t0) t0 = t; }
+            }
+            int idx[3], step[3];
+            double tmax[3], tdel[3];
+            for (int a = 0; a < 3; ++a) {
+                double p = spos[a] + t0 * u[a];
+                int ii = (int)floor((p - lo[a]) / del[a]);
+                if (ii < 0) ii = 0;
+                if (ii > nn[a] - 1) ii = nn[a] - 1;
+                idx[a] = ii;
+                if (u[a] > 0.0) { step[a] = 1; tmax[a] = (lo[a] + (ii + 1) * del[a] - spos[a]) / u[a]; tdel[a] = del[a] / u[a]; }
+                else if (u[a] < 0.0) { step[a] = -1; tmax[a] = (lo[a] + ii * del[a] - spos[a]) / u[a]; tdel[a] = -del[a] / u[a]; }
+                else { step[a] = 0; tmax[a] = INFINITY; tdel[a] = INFINITY; }
+            }
+            double t = t0;
+            for (int it = 0; it < nx + ny + nz + 4 && t < R; ++it) {
+                int a = 0;
+                if (tmax[1] < tmax[a]) a = 1;
+                if (tmax[2] < tmax[a]) a = 2;
+                double tn = tmax[a] < R ? tmax[a] : R;
+                size_t v = (size_t)idx[0] + (size_t)nx * (idx[1] + (size_t)ny * idx[2]);
+                if (tn > t) A[mat[v]] += rho[v] * (tn - t);
+                t = tn;
+                idx[a] += step[a];
+                tmax[a] += tdel[a];
+                if (idx[a] < 0 || idx[a] >= nn[a]) break;
+            }
+        }
+        for (int m = 0; m < n_mat && areal; ++m) areal[(size_t)m * cells + c] = A[m];
+        for (int g = 0; g < G; ++g) {
+            double tau = 0.0;
+            for (int m = 0; m < n_mat; ++m) tau += sigt_hat[(size_t)m * G + g] * A[m];
+            phi_u[(size_t)g * cells + c] = lit ? spectrum[g] * exp(-tau) / (4.0 * M_PI * R2) : 0.0;
+        }
+    }
+}

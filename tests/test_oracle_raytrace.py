@@ -1,0 +1,141 @@
+"""Pins for the oracle's uncollided-flux ray tracer (Eq. 4; readings R11, R12)
+and for the first-collision source (Eq. 5)."""
+import math
+
+import numpy as np
+import pytest
+
+from workloads import Workload, SourceSpec, make_config
+
+
+def _homog(nx, ny, nz, d, rho, sig, G=2):
+    mat = np.zeros((nz, ny, nx), dtype=np.uint8)
+    den = np.full((nz, ny, nx), rho, dtype=np.float32)
+    st = np.array([[sig * (g + 1) for g in range(G)]])
+    ss = np.zeros((1, 1, G, G))
+    return Workload("homog", nx, ny, nz, d[0], d[1], d[2], mat, den, 1, G, 0, 2, st, ss)
+
+
+def _inmesh_length(wl, pos):
+    """In-mesh length of the segment source -> cell centre (slab clipping, numpy)."""
+    lo = -0.5 * np.array([wl.nx * wl.dx, wl.ny * wl.dy, wl.nz * wl.dz]); hi = -lo
+    x = (np.arange(wl.nx) + 0.5) * wl.dx + lo[0]
+    y = (np.arange(wl.ny) + 0.5) * wl.dy + lo[1]
+    z = (np.arange(wl.nz) + 0.5) * wl.dz + lo[2]
+    Z, Y, X = np.meshgrid(z, y, x, indexing="ij")
+    rc = np.stack([X, Y, Z], -1).reshape(-1, 3)
+    d = rc - np.array(pos)
+    R = np.linalg.norm(d, axis=1)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        ta = (lo - np.array(pos)) / d
+        tb = (hi - np.array(pos)) / d
+    tnear = np.nanmax(np.minimum(ta, tb), axis=1)
+    return (1.0 - np.clip(tnear, 0.0, 1.0)) * R, R
+
+
+def test_homogeneous_closed_form(orc):
+    wl = _homog(9, 7, 5, (0.5, 0.6, 0.7), 1.3, 0.4)
+    src = SourceSpec(kind=1, pos=(-6.1, 1.05, 0.33), spectrum=np.array([0.25, 0.75]))
+    phi_u, areal = orc.raytrace(wl, src, want_areal=True)
+    lin, R = _inmesh_length(wl, src.pos)
+    rho = float(np.float32(1.3))
+    assert np.abs(areal[0] / rho - lin).max() < 1e-12              # sum A_m / rho_m = in-mesh length
+    for g in range(2):
+        want = src.spectrum[g] * np.exp(-0.4 * (g + 1) * rho * lin) / (4 * math.pi * R ** 2)
+        assert np.abs(phi_u[g] / want - 1).max() < 1e-12
+
+
+def test_source_inside_mesh(orc):
+    wl = _homog(8, 8, 8, (1.0, 1.0, 1.0), 1.0, 0.3, G=1)
+    src = SourceSpec(kind=1, pos=(0.21, -0.37, 0.11), spectrum=np.array([1.0]))
+    phi_u = orc.raytrace(wl, src)
+    lin, R = _inmesh_length(wl, src.pos)
+    assert np.abs(lin - R).max() < 1e-12
+    assert np.abs(phi_u[0] / (np.exp(-0.3 * R) / (4 * math.pi * R ** 2)) - 1).max() < 1e-12
+
+
+def test_cone_mask(orc):
+    wl = _homog(10, 10, 10, (1.0, 1.0, 1.0), 1.0, 0.1, G=1)
+    pos, axis, half = (-20.0, 0.0, 0.0), (2.0, 0.0, 0.0), math.radians(15.0)
+    a = orc.raytrace(wl, SourceSpec(kind=1, pos=pos, spectrum=np.array([1.0])))
+    b = orc.raytrace(wl, SourceSpec(kind=2, pos=pos, axis=axis, half_angle=half, spectrum=np.array([1.0])))
+    u = orc.unit_dirs_from(wl, pos)
+    inside = u[:, 0] >= math.cos(half)
+    assert 0 < inside.sum() < inside.size
+    assert np.array_equal(b[0][inside], a[0][inside]) and (b[0][~inside] == 0).all()   # hard edge, 4 pi kept (R12)
+
+
+def test_heterogeneous_against_brute_force_sampling(orc):
+    """Optical depth through the config-1 sphere phantom vs a dumb midpoint-rule path integral."""
+    wl = make_config(1)
+    src = wl.sources[0]
+    phi_u, areal = orc.raytrace(wl, src, want_areal=True)
+    rho = wl.density.astype(float).reshape(-1)
+    mat = wl.material.reshape(-1)
+    lo = -0.5 * wl.nx * wl.dx
+    rng = np.random.default_rng(0)
+    for c in rng.integers(0, wl.cells, 25):
+        i, j, k = c % wl.nx, (c // wl.nx) % wl.ny, c // (wl.nx * wl.ny)
+        rc = np.array([lo + (i + 0.5) * wl.dx, lo + (j + 0.5) * wl.dy, lo + (k + 0.5) * wl.dz])
+        n = 400000
+        t = (np.arange(n) + 0.5) / n
+        p = np.array(src.pos)[None, :] + t[:, None] * (rc - np.array(src.pos))[None, :]
+        idx = np.floor((p - lo) / wl.dx).astype(int)
+        ok = ((idx >= 0) & (idx < wl.nx)).all(1)
+        cc = idx[ok, 0] + wl.nx * (idx[ok, 1] + wl.ny * idx[ok, 2])
+        R = np.linalg.norm(rc - np.array(src.pos))
+        for m in range(wl.n_materials):
+            a = (rho[cc] * (mat[cc] == m)).sum() * R / n
+            assert abs(a - areal[m, c]) < 2e-4 * max(1.0, areal[:, c].sum()) + 1e-5
+    # decreasing flux behind the sphere: the shadowed far side is darker than the same distance off-axis
+    g = 10
+    p = phi_u[g].reshape(32, 32, 32)
+    assert p[16, 16, 31] < p[16, 2, 31]
+
+
+def test_first_collision_source_is_eq5(orc):
+    """Eq. (5): S_u(Omega) = int sigma_s(Omega . Omega') phi_u delta(Omega' - u) dOmega'
+    = sum_l (2l+1)/(4pi) sigma_s,l P_l(Omega . u) phi_u.  The oracle forms it as moments
+    rho s_l phi_u Y_lm(u); projected back on the quadrature both must agree (pure scatter group 0)."""
+    from numpy.polynomial import legendre
+    wl = make_config(1)
+    wl.fixed_iters = 1
+    wl.G = 1
+    wl.sigma_t = wl.sigma_t[:, :1].copy(); wl.sigma_s = wl.sigma_s[:, :, :1, :1].copy()
+    wl.sources[0].spectrum = np.array([1.0])
+    res = orc.solve(wl, closure=0)
+    om, w = res["omega"], res["w"]
+    Mtab, _ = orc.projection_tables(3, om, w)
+    # reconstruct the oracle's fixed source from its own definition of the iteration: first sweep has phi = 0,
+    # so Q = fixed; rebuild it here directly from Eq. (5)
+    u = orc.unit_dirs_from(wl, wl.sources[0].pos)
+    rho = wl.density.astype(float).reshape(-1)
+    mat = wl.material.reshape(-1)
+    phi_u = res["phi_u"][0, 0]
+    cells = np.array([5, 1000, 16 + 32 * (16 + 32 * 16), 32767])
+    qn_direct = np.zeros((len(w), len(cells)))
+    for l in range(4):
+        pl = legendre.legval(om @ u[cells].T, [0] * l + [1])
+        qn_direct += (2 * l + 1) / (4 * math.pi) * (rho * wl.sigma_s[mat, l, 0, 0] * phi_u)[cells][None, :] * pl
+    Yu = orc.real_sph_harm(3, u[cells])
+    ll = orc.l_of_lm(3)
+    fixed = (rho * phi_u)[cells][:, None] * wl.sigma_s[mat[cells]][:, ll, 0, 0] * Yu       # [cells][nm]
+    assert np.abs(Mtab @ fixed.T - qn_direct).max() < 1e-13 * np.abs(qn_direct).max()
+
+
+def test_total_balance_with_first_collision_source(orc):
+    """One group, converged: photons scattered out of the uncollided beam = collided absorption + leakage."""
+    wl = make_config(1)
+    wl.G = 1
+    wl.sigma_t = wl.sigma_t[:, 9:10].copy(); wl.sigma_s = wl.sigma_s[:, :, 9:10, 9:10].copy()
+    wl.sources[0].spectrum = np.array([1.0])
+    wl.tol = 1e-10
+    res = orc.solve(wl, closure=0)
+    rho = wl.density.astype(float).reshape(-1); mat = wl.material.reshape(-1)
+    V = wl.dx * wl.dy * wl.dz
+    sig_t = rho * wl.sigma_t[mat, 0]; sig_s0 = rho * wl.sigma_s[mat, 0, 0, 0]
+    first = (sig_s0 * res["phi_u"][0, 0]).sum() * V
+    phi0 = res["phi"][0, 0, 0]
+    absorbed = ((sig_t - sig_s0) * phi0).sum() * V
+    leak = res["balance"][0, 0, 2]
+    assert abs(first - absorbed - leak) < 1e-8 * first
