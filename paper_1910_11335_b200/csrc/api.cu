@@ -1,0 +1,1020 @@
+// C ABI of the B200-native DOCTORS hot path (include/doctors_b200.h): host state machine,
+// workspace planning, launch sequencing.  Every arithmetic step of the path runs in the
+// kernels of kernels.cuh / sweep_brick.cuh; this file only validates, lays out memory and
+// enqueues work on the caller's stream.
+#include "../../include/doctors_b200.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "device_common.cuh"
+#include "host_tables.h"
+#include "kernels.cuh"
+#include "sweep_brick.cuh"
+
+using namespace doctors;
+
+namespace {
+
+struct SourceHost {
+    int kind = 0;
+    double pos[3] = {0, 0, 0}, axis[3] = {1, 0, 0}, half = 0;
+    std::vector<double> spectrum;
+    std::vector<float> volume;
+};
+
+struct GroupResult { int iters; int hit_max; float resid; float pad; double leak; double bal_src; double bal_col; };
+
+// Workspace layout for one choice of options.
+struct Plan {
+    bool ok = false;
+    int px = 0; long long cells_p = 0;
+    int nprob = 0, chunk = 0, nchunks = 0, nsrc = 0, nvol = 0;
+    int G = 0, L = 0, NM = 0, ndir = 0, M = 0;
+    int mode = 0, sweep_mode = 0, deterministic = 0;
+    int B[3] = {0, 0, 0}, gb[3] = {0, 0, 0};
+    long long nbricks = 0, ntasks = 0;
+    size_t smem = 0;
+    // offsets
+    size_t o_mat, o_rho, o_sigt_hat, o_sigs, o_spec, o_srcs, o_extvol, o_mtab, o_dtab, o_dir, o_lk,
+        o_sigt, o_Q, o_fixed, o_phi0old, o_phiall, o_phi0all, o_phiu, o_state, o_ctl, o_leak, o_bal,
+        o_results, o_fixediters, o_tasks, o_flags, o_fx, o_fy, o_fz, o_btab, o_bplane, o_sched, o_ox, o_oy, o_oz;
+    size_t face_x_n = 0, face_y_n = 0, face_z_n = 0;
+    size_t total = 0;
+};
+
+}  // namespace
+
+struct doctors_problem {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    int num_sms = 0;
+    std::string err;
+    // inputs (copied)
+    bool has_mesh = false, has_xs = false, has_quad = false, has_src = false;
+    int nx = 0, ny = 0, nz = 0, n_mat_mesh = 0;
+    double dx = 0, dy = 0, dz = 0;
+    std::vector<uint8_t> mat;
+    std::vector<float> rho;
+    int n_mat_xs = 0, G = 0, L = 0;
+    std::vector<double> sigt, sigs;
+    int ndir = 0;
+    std::vector<double> omega, w;
+    int mode = 0;
+    std::vector<SourceHost> sources;
+    // workspace
+    void* ws = nullptr;
+    size_t ws_bytes = 0;
+    // result bookkeeping
+    bool solved = false;
+    Plan plan;
+    int last_chunk_first = 0, last_chunk_count = 0;
+    CUresult (*encode)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                       const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                       CUtensorMapL2promotion, CUtensorMapFloatOOBfill) = nullptr;
+};
+
+namespace {
+
+int fail(doctors_problem* p, int code, const char* fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (p) p->err = buf;
+    return code;
+}
+
+#define CK(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(p, DOCTORS_CUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+    } while (0)
+
+int nprob_of(const doctors_problem* p) { return p->mode == 0 ? int(p->sources.size()) : 1; }
+
+void auto_brick(int NM, int M, int nx, int ny, int nz, const int* req, int B[3])
+{
+    if (req && req[0] > 0 && req[1] > 0 && req[2] > 0) { B[0] = req[0]; B[1] = req[1]; B[2] = req[2]; return; }
+    const int cand[4][3] = {{8, 8, 8}, {8, 8, 4}, {8, 4, 4}, {4, 4, 4}};
+    for (int c = 0; c < 4; ++c) {
+        B[0] = cand[c][0]; B[1] = cand[c][1]; B[2] = cand[c][2];
+        if (brick_smem_layout(NM, B[0], B[1], B[2], M).total <= 75 * 1024) break;
+    }
+    // do not make bricks larger than the mesh needs
+    B[0] = std::min(B[0], (nx + 3) / 4 * 4);
+    B[1] = std::min(B[1], ny);
+    B[2] = std::min(B[2], nz);
+}
+
+// Lay out the workspace.  chunk = problems solved together.
+Plan make_plan(const doctors_problem* p, const doctors_solve_opts* o, int chunk)
+{
+    Plan P;
+    P.px = (p->nx + 3) / 4 * 4;
+    P.cells_p = (long long)P.px * p->ny * p->nz;
+    P.nprob = nprob_of(p);
+    P.nsrc = int(p->sources.size());
+    P.chunk = std::max(1, std::min(chunk, P.nprob));
+    P.nchunks = (P.nprob + P.chunk - 1) / P.chunk;
+    P.G = p->G; P.L = p->L; P.NM = (p->L + 1) * (p->L + 1);
+    P.ndir = p->ndir; P.M = p->ndir / 8;
+    P.mode = p->mode;
+    P.sweep_mode = o ? o->sweep_mode : 0;
+    P.deterministic = o ? o->deterministic : 0;
+    for (auto& s : p->sources) if (s.kind == 0) ++P.nvol;
+    auto_brick(P.NM, P.M, p->nx, p->ny, p->nz, o ? o->brick : nullptr, P.B);
+    P.gb[0] = (p->nx + P.B[0] - 1) / P.B[0];
+    P.gb[1] = (p->ny + P.B[1] - 1) / P.B[1];
+    P.gb[2] = (p->nz + P.B[2] - 1) / P.B[2];
+    P.nbricks = (long long)P.gb[0] * P.gb[1] * P.gb[2];
+    P.ntasks = P.nbricks * 8 * P.chunk;
+    P.smem = brick_smem_layout(P.NM, P.B[0], P.B[1], P.B[2], P.M).total;
+
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t r = off; off = align_up(off + bytes, 256); return r; };
+    const size_t cp = size_t(P.cells_p), nm = size_t(P.NM), G = size_t(P.G);
+    // the memory in a mode-1 chunk: sources of the chunk = all sources
+    const size_t src_per_chunk = P.mode == 0 ? size_t(P.chunk) : size_t(P.nsrc);
+    (void)src_per_chunk;
+    P.o_mat = take(cp);
+    P.o_rho = take(cp * 4);
+    P.o_sigt_hat = take(size_t(p->n_mat_xs) * G * 8);
+    P.o_sigs = take(size_t(p->n_mat_xs) * (P.L + 1) * G * G * 4);
+    P.o_spec = take(size_t(P.nsrc) * G * 8);
+    P.o_srcs = take(size_t(P.nsrc) * sizeof(SourceDev));
+    P.o_extvol = take(size_t(P.nvol) * G * cp * 4);
+    P.o_mtab = take(size_t(P.ndir) * nm * 4);
+    P.o_dtab = take(size_t(P.ndir) * nm * 4);
+    P.o_dir = take(size_t(P.ndir) * 16);
+    P.o_lk = take(size_t(P.ndir) * 16);
+    P.o_sigt = take(cp * 4);
+    P.o_Q = take(size_t(P.chunk) * nm * cp * 4);
+    P.o_fixed = take(size_t(P.chunk) * nm * cp * 4);
+    P.o_phi0old = take(size_t(P.chunk) * cp * 4);
+    P.o_phiall = take(size_t(P.chunk) * G * nm * cp * 4);
+    P.o_phi0all = take(size_t(P.nprob) * G * cp * 4);
+    P.o_phiu = take(size_t(P.nsrc) * G * cp * 4);
+    P.o_state = take(size_t(P.chunk) * sizeof(ProbState));
+    P.o_ctl = take(sizeof(Control));
+    P.o_leak = take(size_t(P.chunk) * 8);
+    P.o_bal = take(size_t(P.chunk) * 16);
+    P.o_results = take(size_t(P.nprob) * G * sizeof(GroupResult));
+    P.o_fixediters = take(size_t(P.nprob) * G * 4);
+    if (P.sweep_mode == 0) {
+        P.face_x_n = size_t(P.M) * P.B[1] * P.B[2];
+        P.face_y_n = size_t(P.M) * P.B[0] * P.B[2];
+        P.face_z_n = size_t(P.M) * P.B[0] * P.B[1];
+        P.o_tasks = take(size_t(P.ntasks) * sizeof(uint2));
+        P.o_flags = take(size_t(P.chunk) * 8 * P.nbricks * 4);
+        P.o_fx = take(size_t(P.chunk) * 8 * P.gb[1] * P.gb[2] * P.face_x_n * 4);
+        P.o_fy = take(size_t(P.chunk) * 8 * P.gb[0] * P.gb[2] * P.face_y_n * 4);
+        P.o_fz = take(size_t(P.chunk) * 8 * P.gb[0] * P.gb[1] * P.face_z_n * 4);
+        P.o_btab = take(size_t(P.B[0]) * P.B[1] * P.B[2] * 4);
+        P.o_bplane = take(size_t(P.B[0] + P.B[1] + P.B[2]) * 4);
+        P.o_sched = P.o_ox = P.o_oy = P.o_oz = 0;
+    } else {
+        P.o_sched = take(size_t(8) * p->nx * p->ny * p->nz * 4);
+        P.o_ox = take(size_t(P.chunk) * P.M * cp * 4);
+        P.o_oy = take(size_t(P.chunk) * P.M * cp * 4);
+        P.o_oz = take(size_t(P.chunk) * P.M * cp * 4);
+        P.o_tasks = P.o_flags = P.o_fx = P.o_fy = P.o_fz = P.o_btab = P.o_bplane = 0;
+    }
+    P.total = off;
+    P.ok = true;
+    return P;
+}
+
+int check_ready(doctors_problem* p)
+{
+    if (!p->has_mesh) return fail(p, DOCTORS_BAD_STATE, "mesh/materials not set");
+    if (!p->has_xs) return fail(p, DOCTORS_BAD_STATE, "cross sections not set");
+    if (!p->has_quad) return fail(p, DOCTORS_BAD_STATE, "quadrature not set");
+    if (!p->has_src) return fail(p, DOCTORS_BAD_STATE, "source not set");
+    if (p->n_mat_mesh > p->n_mat_xs)
+        return fail(p, DOCTORS_BAD_STATE, "mesh uses %d materials, XS table has %d", p->n_mat_mesh, p->n_mat_xs);
+    for (size_t s = 0; s < p->sources.size(); ++s) {
+        const SourceHost& S = p->sources[s];
+        if (S.kind == 0) {
+            if (S.volume.size() != size_t(p->G) * p->nx * p->ny * p->nz)
+                return fail(p, DOCTORS_BAD_STATE, "source %zu: volume array does not match G x mesh", s);
+        } else if (S.spectrum.size() != size_t(p->G)) {
+            return fail(p, DOCTORS_BAD_STATE, "source %zu: spectrum length %zu != G = %d", s, S.spectrum.size(), p->G);
+        }
+    }
+    return DOCTORS_OK;
+}
+
+// choose the chunk: the option, or the largest balanced chunk that fits `budget` bytes
+int choose_chunk(const doctors_problem* p, const doctors_solve_opts* o, size_t budget)
+{
+    int nprob = nprob_of(p);
+    if (o && o->source_chunk > 0) return std::min(o->source_chunk, nprob);
+    int best = 1;
+    for (int c = 1; c <= nprob; ++c)
+        if (make_plan(p, o, c).total <= budget) best = c;
+    int nch = (nprob + best - 1) / best;
+    return (nprob + nch - 1) / nch;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------
+extern "C" {
+
+const char* doctors_version(void) { return "doctors-b200 0.1 (sm_100a)"; }
+
+int doctors_create_problem(int cuda_device, void* stream, doctors_problem** out)
+{
+    if (!out) return DOCTORS_INVALID_ARG;
+    *out = nullptr;
+    int n = 0;
+    cudaError_t e = cudaGetDeviceCount(&n);
+    if (e != cudaSuccess || n <= 0 || cuda_device < 0 || cuda_device >= n) return DOCTORS_CUDA;
+    if (cudaSetDevice(cuda_device) != cudaSuccess) return DOCTORS_CUDA;
+    doctors_problem* p = new (std::nothrow) doctors_problem();
+    if (!p) return DOCTORS_ALLOC;
+    p->device = cuda_device;
+    p->stream = static_cast<cudaStream_t>(stream);
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess) { delete p; return DOCTORS_CUDA; }
+    p->num_sms = prop.multiProcessorCount;
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess ||
+        qres != cudaDriverEntryPointSuccess || !fn) { delete p; return DOCTORS_CUDA; }
+    p->encode = reinterpret_cast<decltype(p->encode)>(fn);
+    *out = p;
+    return DOCTORS_OK;
+}
+
+void doctors_destroy_problem(doctors_problem* p) { delete p; }
+
+const char* doctors_last_error(const doctors_problem* p) { return p ? p->err.c_str() : "null handle"; }
+
+int doctors_set_mesh_materials(doctors_problem* p, int nx, int ny, int nz, double dx, double dy, double dz,
+                               const uint8_t* material_id, const float* density, int n_materials)
+{
+    if (!p) return DOCTORS_INVALID_ARG;
+    if (nx <= 0 || ny <= 0 || nz <= 0) return fail(p, DOCTORS_INVALID_ARG, "mesh extents must be positive");
+    if (!(dx > 0 && dy > 0 && dz > 0) || !std::isfinite(dx) || !std::isfinite(dy) || !std::isfinite(dz))
+        return fail(p, DOCTORS_INVALID_ARG, "voxel pitch must be positive and finite");
+    if (!material_id) return fail(p, DOCTORS_INVALID_ARG, "material_id is NULL");
+    if (n_materials <= 0 || n_materials > kMaxMaterials)
+        return fail(p, DOCTORS_INVALID_ARG, "n_materials must be 1..%d", kMaxMaterials);
+    if ((long long)nx * ny * nz > (1LL << 30)) return fail(p, DOCTORS_INVALID_ARG, "mesh too large");
+    size_t cells = size_t(nx) * ny * nz;
+    for (size_t c = 0; c < cells; ++c) {
+        if (material_id[c] >= n_materials) return fail(p, DOCTORS_INVALID_ARG, "material id %d >= n_materials at cell %zu", int(material_id[c]), c);
+        if (density && !(density[c] >= 0.0f && std::isfinite(density[c])))
+            return fail(p, DOCTORS_INVALID_ARG, "density must be finite and >= 0 (cell %zu)", c);
+    }
+    p->nx = nx; p->ny = ny; p->nz = nz; p->dx = dx; p->dy = dy; p->dz = dz;
+    p->n_mat_mesh = n_materials;
+    p->mat.assign(material_id, material_id + cells);
+    if (density) p->rho.assign(density, density + cells); else p->rho.assign(cells, 1.0f);
+    p->has_mesh = true;
+    p->solved = false;
+    return DOCTORS_OK;
+}
+
+int doctors_set_xs(doctors_problem* p, int n_materials, int n_groups, int pl_order, const double* sigma_t, const double* sigma_s)
+{
+    if (!p) return DOCTORS_INVALID_ARG;
+    if (n_materials <= 0 || n_materials > kMaxMaterials) return fail(p, DOCTORS_INVALID_ARG, "n_materials must be 1..%d", kMaxMaterials);
+    if (n_groups <= 0 || n_groups > 4096) return fail(p, DOCTORS_INVALID_ARG, "n_groups must be 1..4096");
+    if (pl_order < 0 || pl_order > 3) return fail(p, DOCTORS_INVALID_ARG, "pl_order must be 0..3");
+    if (!sigma_t || !sigma_s) return fail(p, DOCTORS_INVALID_ARG, "NULL table");
+    const int G = n_groups, L = pl_order;
+    for (int m = 0; m < n_materials; ++m)
+        for (int g = 0; g < G; ++g)
+            if (!(sigma_t[m * G + g] >= 0.0) || !std::isfinite(sigma_t[m * G + g]))
+                return fail(p, DOCTORS_INVALID_ARG, "sigma_t[%d][%d] must be finite and >= 0", m, g);
+    for (int m = 0; m < n_materials; ++m)
+        for (int l = 0; l <= L; ++l)
+            for (int gf = 0; gf < G; ++gf)
+                for (int gt = 0; gt < G; ++gt) {
+                    double v = sigma_s[((size_t(m) * (L + 1) + l) * G + gf) * G + gt];
+                    if (!std::isfinite(v)) return fail(p, DOCTORS_INVALID_ARG, "sigma_s not finite");
+                    if (gt < gf && v != 0.0)
+                        return fail(p, DOCTORS_INVALID_ARG, "upscatter entry sigma_s[%d][%d][%d->%d] != 0 (downscatter only, PAPER.md:34)", m, l, gf, gt);
+                }
+    p->n_mat_xs = n_materials; p->G = G; p->L = L;
+    p->sigt.assign(sigma_t, sigma_t + size_t(n_materials) * G);
+    p->sigs.assign(sigma_s, sigma_s + size_t(n_materials) * (L + 1) * G * G);
+    p->has_xs = true;
+    p->solved = false;
+    return DOCTORS_OK;
+}
+
+int doctors_set_quadrature(doctors_problem* p, int sn_order)
+{
+    if (!p) return DOCTORS_INVALID_ARG;
+    std::vector<double> om, w;
+    if (!level_symmetric(sn_order, om, w))
+        return fail(p, DOCTORS_INVALID_ARG, "S_N order must be one of 2, 4, 6, 8, 12, 16");
+    p->omega = om; p->w = w; p->ndir = int(w.size());
+    p->has_quad = true;
+    p->solved = false;
+    return DOCTORS_OK;
+}
+
+int doctors_set_quadrature_points(doctors_problem* p, int n_dir, const double* omega_xyz, const double* w)
+{
+    if (!p) return DOCTORS_INVALID_ARG;
+    if (n_dir <= 0 || n_dir % 8 != 0 || !omega_xyz || !w) return fail(p, DOCTORS_INVALID_ARG, "n_dir must be a positive multiple of 8");
+    if (n_dir / 8 > 64) return fail(p, DOCTORS_INVALID_ARG, "at most 64 directions per octant");
+    double sw = 0.0;
+    std::vector<std::vector<int>> by_oct(8);
+    const double pi = std::acos(-1.0);
+    for (int n = 0; n < n_dir; ++n) {
+        const double* o = omega_xyz + 3 * n;
+        double nr = std::sqrt(o[0] * o[0] + o[1] * o[1] + o[2] * o[2]);
+        if (std::fabs(nr - 1.0) > 1e-10) return fail(p, DOCTORS_INVALID_ARG, "direction %d is not a unit vector", n);
+        if (o[0] == 0.0 || o[1] == 0.0 || o[2] == 0.0) return fail(p, DOCTORS_INVALID_ARG, "direction %d has a zero component", n);
+        if (!(w[n] > 0.0)) return fail(p, DOCTORS_INVALID_ARG, "weight %d must be positive", n);
+        sw += w[n];
+        by_oct[(o[0] < 0 ? 1 : 0) | (o[1] < 0 ? 2 : 0) | (o[2] < 0 ? 4 : 0)].push_back(n);
+    }
+    if (std::fabs(sw - 4.0 * pi) > 1e-10 * 4.0 * pi) return fail(p, DOCTORS_INVALID_ARG, "weights sum to %.15g, not 4 pi", sw);
+    for (int o = 0; o < 8; ++o)
+        if (int(by_oct[o].size()) != n_dir / 8) return fail(p, DOCTORS_INVALID_ARG, "octant %d has %zu directions, expected %d", o, by_oct[o].size(), n_dir / 8);
+    p->omega.clear(); p->w.clear();
+    for (int o = 0; o < 8; ++o)
+        for (int n : by_oct[o]) {
+            p->omega.insert(p->omega.end(), omega_xyz + 3 * n, omega_xyz + 3 * n + 3);
+            p->w.push_back(w[n]);
+        }
+    p->ndir = n_dir;
+    p->has_quad = true;
+    p->solved = false;
+    return DOCTORS_OK;
+}
+
+int doctors_get_quadrature(const doctors_problem* p, int* n_dir, double* omega_xyz, double* w)
+{
+    if (!p || !n_dir) return DOCTORS_INVALID_ARG;
+    if (!p->has_quad) return DOCTORS_BAD_STATE;
+    *n_dir = p->ndir;
+    if (omega_xyz) std::memcpy(omega_xyz, p->omega.data(), p->omega.size() * 8);
+    if (w) std::memcpy(w, p->w.data(), p->w.size() * 8);
+    return DOCTORS_OK;
+}
+
+int doctors_set_source(doctors_problem* p, int n_sources, const doctors_source* src, int mode)
+{
+    if (!p) return DOCTORS_INVALID_ARG;
+    if (n_sources <= 0 || n_sources > 64 || !src) return fail(p, DOCTORS_INVALID_ARG, "n_sources must be 1..64");
+    if (mode != 0 && mode != 1) return fail(p, DOCTORS_INVALID_ARG, "mode must be 0 or 1");
+    if (!p->has_mesh || !p->has_xs) return fail(p, DOCTORS_BAD_STATE, "set the mesh and the cross sections before the source (array lengths)");
+    std::vector<SourceHost> v(n_sources);
+    const size_t cells = size_t(p->nx) * p->ny * p->nz;
+    for (int s = 0; s < n_sources; ++s) {
+        const doctors_source& S = src[s];
+        SourceHost& H = v[s];
+        H.kind = S.kind;
+        if (S.kind == 0) {
+            if (!S.volume) return fail(p, DOCTORS_INVALID_ARG, "source %d: volume is NULL", s);
+            H.volume.assign(S.volume, S.volume + size_t(p->G) * cells);
+            for (float f : H.volume) if (!std::isfinite(f)) return fail(p, DOCTORS_INVALID_ARG, "source %d: volume not finite", s);
+        } else if (S.kind == 1 || S.kind == 2) {
+            if (!S.spectrum) return fail(p, DOCTORS_INVALID_ARG, "source %d: spectrum is NULL", s);
+            H.spectrum.assign(S.spectrum, S.spectrum + p->G);
+            for (int a = 0; a < 3; ++a) { H.pos[a] = S.pos[a]; H.axis[a] = S.axis[a]; }
+            H.half = S.half_angle_rad;
+            if (S.kind == 2) {
+                double an = std::sqrt(S.axis[0] * S.axis[0] + S.axis[1] * S.axis[1] + S.axis[2] * S.axis[2]);
+                if (!(an > 0.0) || !(S.half_angle_rad > 0.0)) return fail(p, DOCTORS_INVALID_ARG, "source %d: cone needs an axis and a half angle", s);
+                for (int a = 0; a < 3; ++a) H.axis[a] = S.axis[a] / an;
+            }
+            // 1/R^2 singularity: a source on a cell centre
+            const double d[3] = {p->dx, p->dy, p->dz};
+            const int nn[3] = {p->nx, p->ny, p->nz};
+            bool on_centre = true;
+            for (int a = 0; a < 3; ++a) {
+                double f = (S.pos[a] + 0.5 * nn[a] * d[a]) / d[a] - 0.5;      // fractional cell index
+                double r = std::round(f);
+                if (!(r >= 0 && r <= nn[a] - 1 && std::fabs(f - r) < 1e-9)) on_centre = false;
+            }
+            if (on_centre) return fail(p, DOCTORS_INVALID_ARG, "source %d sits on a cell centre (1/R^2 singularity)", s);
+        } else {
+            return fail(p, DOCTORS_INVALID_ARG, "source %d: unknown kind %d", s, S.kind);
+        }
+    }
+    p->sources.swap(v);
+    p->mode = mode;
+    p->has_src = true;
+    p->solved = false;
+    return DOCTORS_OK;
+}
+
+int doctors_n_problems(const doctors_problem* p) { return p && p->has_src ? nprob_of(p) : 0; }
+
+size_t doctors_workspace_bytes(doctors_problem* p, const doctors_solve_opts* opts)
+{
+    if (!p) return 0;
+    if (check_ready(p) != DOCTORS_OK) return 0;
+    size_t fr = 0, tot = 0;
+    cudaSetDevice(p->device);
+    if (cudaMemGetInfo(&fr, &tot) != cudaSuccess) { fail(p, DOCTORS_CUDA, "cudaMemGetInfo failed"); return 0; }
+    int chunk = choose_chunk(p, opts, size_t(double(fr) * 0.85));
+    return make_plan(p, opts, chunk).total;
+}
+
+int doctors_set_workspace(doctors_problem* p, void* device_ptr, size_t bytes)
+{
+    if (!p) return DOCTORS_INVALID_ARG;
+    if (!device_ptr || (reinterpret_cast<uintptr_t>(device_ptr) & 255u)) return fail(p, DOCTORS_INVALID_ARG, "workspace must be non-NULL and 256-byte aligned");
+    p->ws = device_ptr; p->ws_bytes = bytes;
+    p->solved = false;
+    return DOCTORS_OK;
+}
+
+long long doctors_wavefront_size(int nx, int ny, int nz, int S) { return wavefront_size(nx, ny, nz, S); }
+
+int doctors_debug_schedule_dims(doctors_problem* p, const doctors_solve_opts* opts, int level, int dims[3])
+{
+    if (!p || !dims) return DOCTORS_INVALID_ARG;
+    if (!p->has_mesh) return fail(p, DOCTORS_BAD_STATE, "mesh not set");
+    if (level == 0) { dims[0] = p->nx; dims[1] = p->ny; dims[2] = p->nz; return DOCTORS_OK; }
+    if (!p->has_xs || !p->has_quad) return fail(p, DOCTORS_BAD_STATE, "xs / quadrature not set (brick size depends on them)");
+    int B[3];
+    auto_brick((p->L + 1) * (p->L + 1), p->ndir / 8, p->nx, p->ny, p->nz, opts ? opts->brick : nullptr, B);
+    if (level == 1) { for (int a = 0; a < 3; ++a) dims[a] = ((a == 0 ? p->nx : a == 1 ? p->ny : p->nz) + B[a] - 1) / B[a]; return DOCTORS_OK; }
+    if (level == 2) { for (int a = 0; a < 3; ++a) dims[a] = B[a]; return DOCTORS_OK; }
+    return fail(p, DOCTORS_INVALID_ARG, "level must be 0, 1 or 2");
+}
+
+int doctors_debug_get_schedule(doctors_problem* p, const doctors_solve_opts* opts, int octant, int level,
+                               int32_t* plane_offset, int32_t* cell_of)
+{
+    if (!p || !plane_offset || !cell_of || octant < 0 || octant > 7) return DOCTORS_INVALID_ARG;
+    int d[3];
+    int rc = doctors_debug_schedule_dims(p, opts, level, d);
+    if (rc != DOCTORS_OK) return rc;
+    std::vector<int32_t> off, cells;
+    subsweep_schedule(d[0], d[1], d[2], octant, off, cells);
+    std::memcpy(plane_offset, off.data(), off.size() * 4);
+    std::memcpy(cell_of, cells.data(), cells.size() * 4);
+    return DOCTORS_OK;
+}
+
+int doctors_debug_get_tables(const doctors_problem* p, int pl_order, double* Mtab, double* Dtab)
+{
+    if (!p || pl_order < 0 || pl_order > 3 || !Mtab || !Dtab) return DOCTORS_INVALID_ARG;
+    if (!p->has_quad) return DOCTORS_BAD_STATE;
+    std::vector<double> M, D;
+    projection_tables(pl_order, p->omega, p->w, M, D);
+    std::memcpy(Mtab, M.data(), M.size() * 8);
+    std::memcpy(Dtab, D.data(), D.size() * 8);
+    return DOCTORS_OK;
+}
+
+int doctors_host_level_symmetric(int sn_order, double* omega_xyz, double* w)
+{
+    std::vector<double> om, ww;
+    if (!omega_xyz || !w || !level_symmetric(sn_order, om, ww)) return DOCTORS_INVALID_ARG;
+    std::memcpy(omega_xyz, om.data(), om.size() * 8);
+    std::memcpy(w, ww.data(), ww.size() * 8);
+    return DOCTORS_OK;
+}
+
+int doctors_host_schedule(int nx, int ny, int nz, int octant, int32_t* plane_offset, int32_t* cell_of)
+{
+    if (nx <= 0 || ny <= 0 || nz <= 0 || octant < 0 || octant > 7 || !plane_offset || !cell_of) return DOCTORS_INVALID_ARG;
+    std::vector<int32_t> off, cells;
+    subsweep_schedule(nx, ny, nz, octant, off, cells);
+    std::memcpy(plane_offset, off.data(), off.size() * 4);
+    std::memcpy(cell_of, cells.data(), cells.size() * 4);
+    return DOCTORS_OK;
+}
+
+int doctors_host_projection_tables(int pl_order, int n_dir, const double* omega_xyz, const double* w, double* Mtab, double* Dtab)
+{
+    if (pl_order < 0 || pl_order > 3 || n_dir <= 0 || !omega_xyz || !w || !Mtab || !Dtab) return DOCTORS_INVALID_ARG;
+    std::vector<double> om(omega_xyz, omega_xyz + 3 * size_t(n_dir)), ww(w, w + n_dir), M, D;
+    projection_tables(pl_order, om, ww, M, D);
+    std::memcpy(Mtab, M.data(), M.size() * 8);
+    std::memcpy(Dtab, D.data(), D.size() * 8);
+    return DOCTORS_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------
+// solve
+// ------------------------------------------------------------------------------------------
+namespace {
+
+__global__ void k_group_begin(ProbState* st, Control* ctl, const int* fixed_iters, int prob0, int n, int chunk, int G, int g, double* bal)
+{
+    int q = threadIdx.x;
+    if (q >= n && q < chunk) st[q].done = 1;          // short last chunk: no such problem
+    if (q < n) {
+        ProbState s;
+        s.max_diff_bits = 0u; s.max_phi_bits = 0u; s.iters = 0; s.done = 0;
+        s.fixed = fixed_iters[(size_t)(prob0 + q) * G + g];
+        s.hit_max = 0; s.resid = 0.0f; s.pad = 0;
+        st[q] = s;
+        bal[2 * q] = 0.0; bal[2 * q + 1] = 0.0;
+    }
+    if (q == 0) { ctl->ticket = 0u; ctl->all_done = 0; }
+}
+
+__global__ void k_group_end(const ProbState* st, const double* leak, const double* bal, GroupResult* res, int prob0, int n, int G, int g)
+{
+    int q = threadIdx.x;
+    if (q < n) {
+        GroupResult r;
+        r.iters = st[q].iters; r.hit_max = st[q].hit_max; r.resid = st[q].resid; r.pad = 0.0f;
+        r.leak = leak[q]; r.bal_src = bal[2 * q]; r.bal_col = bal[2 * q + 1];
+        res[(size_t)(prob0 + q) * G + g] = r;
+    }
+}
+
+// copy the scalar flux of the finished group into the retained array
+__global__ void k_keep_phi0(long long cells_p, int g, int G, int NM, const float* __restrict__ phi_all,
+                            float* __restrict__ phi0_all, int prob0)
+{
+    const int q = blockIdx.y;
+    const float* src = phi_all + ((size_t)q * G + g) * NM * cells_p;
+    float* dst = phi0_all + ((size_t)(prob0 + q) * G + g) * cells_p;
+    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < cells_p; c += (long long)gridDim.x * blockDim.x)
+        dst[c] = src[c];
+}
+
+template <typename T>
+T* at(doctors_problem* p, size_t off) { return reinterpret_cast<T*>(static_cast<char*>(p->ws) + off); }
+
+int make_tensor_map(doctors_problem* p, CUtensorMap* tm, void* base, int rank, const cuuint64_t* dims,
+                    const cuuint64_t* strides_bytes /*rank-1*/, const cuuint32_t* box)
+{
+    cuuint32_t es[5] = {1, 1, 1, 1, 1};
+    CUresult r = p->encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, cuuint32_t(rank), base, dims, strides_bytes, box, es,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                           CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(p, DOCTORS_CUDA, "cuTensorMapEncodeTiled failed (%d)", int(r));
+    return DOCTORS_OK;
+}
+
+struct SweepLaunch {
+    CUtensorMap tmQ, tmPhi, tmSig;
+    BrickParams bp;
+    int grid = 0;
+    size_t smem = 0;
+};
+
+template <int NM, bool FIX>
+cudaError_t launch_brick(const SweepLaunch& S, cudaStream_t st)
+{
+    k_sweep_brick<NM, FIX><<<S.grid, kSweepThreads, S.smem, st>>>(S.tmQ, S.tmPhi, S.tmSig, S.bp);
+    return cudaGetLastError();
+}
+
+template <int NM, bool FIX>
+cudaError_t prep_brick(size_t smem, int* max_ctas)
+{
+    cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<NM, FIX>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+    if (e != cudaSuccess) return e;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(max_ctas, k_sweep_brick<NM, FIX>, kSweepThreads, smem);
+}
+
+#define DISPATCH_NM_FIX(NMv, FIXv, EXPR)                                         \
+    do {                                                                         \
+        if (FIXv) {                                                              \
+            switch (NMv) {                                                       \
+                case 1: { constexpr int NM = 1; constexpr bool FIX = true; EXPR; } break;   \
+                case 4: { constexpr int NM = 4; constexpr bool FIX = true; EXPR; } break;   \
+                case 9: { constexpr int NM = 9; constexpr bool FIX = true; EXPR; } break;   \
+                default: { constexpr int NM = 16; constexpr bool FIX = true; EXPR; } break; \
+            }                                                                    \
+        } else {                                                                 \
+            switch (NMv) {                                                       \
+                case 1: { constexpr int NM = 1; constexpr bool FIX = false; EXPR; } break;  \
+                case 4: { constexpr int NM = 4; constexpr bool FIX = false; EXPR; } break;  \
+                case 9: { constexpr int NM = 9; constexpr bool FIX = false; EXPR; } break;  \
+                default: { constexpr int NM = 16; constexpr bool FIX = false; EXPR; } break;\
+            }                                                                    \
+        }                                                                        \
+    } while (0)
+
+}  // namespace
+
+extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_in, doctors_solve_info* info)
+{
+    if (!p) return DOCTORS_INVALID_ARG;
+    int rc = check_ready(p);
+    if (rc != DOCTORS_OK) return rc;
+    doctors_solve_opts o;
+    std::memset(&o, 0, sizeof o);
+    if (opts_in) o = *opts_in;
+    if (!(o.tol > 0.0)) o.tol = 1e-5;
+    if (o.max_iters <= 0) o.max_iters = 100;
+    if (o.check_window <= 0) o.check_window = 12;
+    if (o.closure != 0 && o.closure != 1) return fail(p, DOCTORS_INVALID_ARG, "closure must be 0 or 1");
+    if (o.sweep_mode != 0 && o.sweep_mode != 1) return fail(p, DOCTORS_INVALID_ARG, "sweep_mode must be 0 or 1");
+    if (o.brick[0] > 0 && (o.brick[0] % 4 != 0 || o.brick[0] > 64 || o.brick[1] > 64 || o.brick[2] > 64 || o.brick[1] <= 0 || o.brick[2] <= 0))
+        return fail(p, DOCTORS_INVALID_ARG, "brick extents must be 1..64 with brick[0] a multiple of 4");
+    if (!p->ws) return fail(p, DOCTORS_ALLOC, "no workspace set");
+    CK(cudaSetDevice(p->device));
+    cudaStream_t st = p->stream;
+
+    const int chunk = choose_chunk(p, &o, p->ws_bytes);
+    Plan P = make_plan(p, &o, chunk);
+    if (P.total > p->ws_bytes)
+        return fail(p, DOCTORS_ALLOC, "workspace too small: need %zu bytes (chunk %d), have %zu", P.total, P.chunk, p->ws_bytes);
+    if (P.chunk > 255) return fail(p, DOCTORS_INVALID_ARG, "chunk too large");
+    if (P.gb[0] > 1023 || P.gb[1] > 1023 || P.gb[2] > 1023) return fail(p, DOCTORS_INVALID_ARG, "brick grid too large");
+    p->solved = false;
+    p->plan = P;
+    const int NM = P.NM, G = P.G, L = P.L, M = P.M;
+    const size_t cp = size_t(P.cells_p);
+    const int nx = p->nx, ny = p->ny, nz = p->nz, px = P.px;
+
+    MeshDev md;
+    md.nx = nx; md.ny = ny; md.nz = nz; md.px = px; md.cells_p = P.cells_p;
+    md.dx = p->dx; md.dy = p->dy; md.dz = p->dz;
+    md.x0 = 0.5 * p->dx - 0.5 * nx * p->dx; md.y0 = 0.5 * p->dy - 0.5 * ny * p->dy; md.z0 = 0.5 * p->dz - 0.5 * nz * p->dz;
+
+    // ---- upload inputs and tables (pitched rows) ----
+    {
+        std::vector<uint8_t> hm(cp, 0);
+        std::vector<float> hr(cp, 0.0f);
+        for (int k = 0; k < nz; ++k)
+            for (int j = 0; j < ny; ++j) {
+                std::memcpy(&hm[(size_t)px * (j + (size_t)ny * k)], &p->mat[(size_t)nx * (j + (size_t)ny * k)], nx);
+                std::memcpy(&hr[(size_t)px * (j + (size_t)ny * k)], &p->rho[(size_t)nx * (j + (size_t)ny * k)], size_t(nx) * 4);
+            }
+        CK(cudaMemcpyAsync(at<uint8_t>(p, P.o_mat), hm.data(), cp, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(at<float>(p, P.o_rho), hr.data(), cp * 4, cudaMemcpyHostToDevice, st));
+        CK(cudaStreamSynchronize(st));
+    }
+    std::vector<float> sigs_f(p->sigs.begin(), p->sigs.end());
+    std::vector<double> spec(size_t(P.nsrc) * G, 0.0);
+    std::vector<SourceDev> sdev(P.nsrc);
+    {
+        int slot = 0;
+        for (int s = 0; s < P.nsrc; ++s) {
+            const SourceHost& H = p->sources[s];
+            SourceDev& D = sdev[s];
+            D.kind = H.kind; D.vol_slot = -1;
+            for (int a = 0; a < 3; ++a) { D.pos[a] = H.pos[a]; D.axis[a] = H.axis[a]; }
+            D.cos_half = std::cos(H.half);
+            if (H.kind == 0) {
+                D.vol_slot = slot;
+                std::vector<float> hv(size_t(G) * cp, 0.0f);
+                for (int g = 0; g < G; ++g)
+                    for (int k = 0; k < nz; ++k)
+                        for (int j = 0; j < ny; ++j)
+                            std::memcpy(&hv[(size_t)g * cp + (size_t)px * (j + (size_t)ny * k)],
+                                        &H.volume[((size_t)g * nz + k) * ny * nx + (size_t)j * nx], size_t(nx) * 4);
+                CK(cudaMemcpyAsync(at<float>(p, P.o_extvol) + (size_t)slot * G * cp, hv.data(), hv.size() * 4, cudaMemcpyHostToDevice, st));
+                CK(cudaStreamSynchronize(st));
+                ++slot;
+            } else {
+                for (int g = 0; g < G; ++g) spec[(size_t)s * G + g] = H.spectrum[g];
+            }
+        }
+    }
+    std::vector<double> Mt, Dt;
+    projection_tables(L, p->omega, p->w, Mt, Dt);
+    std::vector<float> Mt_f(Mt.begin(), Mt.end()), Dt_f(Dt.begin(), Dt.end());
+    std::vector<float4> dirc(P.ndir), lkc(P.ndir);
+    for (int n = 0; n < P.ndir; ++n) {
+        double cx = 2.0 * std::fabs(p->omega[3 * n]) / p->dx, cy = 2.0 * std::fabs(p->omega[3 * n + 1]) / p->dy, cz = 2.0 * std::fabs(p->omega[3 * n + 2]) / p->dz;
+        dirc[n] = make_float4(float(cx), float(cy), float(cz), float(cx + cy + cz));
+        lkc[n] = make_float4(float(p->w[n] * std::fabs(p->omega[3 * n]) * p->dy * p->dz),
+                             float(p->w[n] * std::fabs(p->omega[3 * n + 1]) * p->dx * p->dz),
+                             float(p->w[n] * std::fabs(p->omega[3 * n + 2]) * p->dx * p->dy), 0.0f);
+    }
+    std::vector<int> fixed_h(size_t(P.nprob) * G, 0);
+    if (o.fixed_iters) std::copy(o.fixed_iters, o.fixed_iters + fixed_h.size(), fixed_h.begin());
+    CK(cudaMemcpyAsync(at<double>(p, P.o_sigt_hat), p->sigt.data(), p->sigt.size() * 8, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(at<float>(p, P.o_sigs), sigs_f.data(), sigs_f.size() * 4, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(at<double>(p, P.o_spec), spec.data(), spec.size() * 8, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(at<SourceDev>(p, P.o_srcs), sdev.data(), sdev.size() * sizeof(SourceDev), cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(at<float>(p, P.o_mtab), Mt_f.data(), Mt_f.size() * 4, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(at<float>(p, P.o_dtab), Dt_f.data(), Dt_f.size() * 4, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(at<float4>(p, P.o_dir), dirc.data(), dirc.size() * 16, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(at<float4>(p, P.o_lk), lkc.data(), lkc.size() * 16, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(at<int>(p, P.o_fixediters), fixed_h.data(), fixed_h.size() * 4, cudaMemcpyHostToDevice, st));
+
+    // ---- schedules (a3) ----
+    std::vector<uint2> tasks;
+    std::vector<int> oct_begin(9, 0);
+    std::vector<std::vector<int32_t>> sched_off(8);
+    SweepLaunch SL;
+    int ctas_per_sm = 0;
+    if (P.sweep_mode == 0) {
+        // level 2: cells of a full brick, sweep-space order (octant 0); the kernel mirrors per octant
+        std::vector<int32_t> boff, bcell;
+        subsweep_schedule(P.B[0], P.B[1], P.B[2], 0, boff, bcell);
+        std::vector<uint32_t> btab(bcell.size());
+        for (size_t t = 0; t < bcell.size(); ++t) {
+            int c = bcell[t];
+            int i = c % P.B[0], j = (c / P.B[0]) % P.B[1], k = c / (P.B[0] * P.B[1]);
+            btab[t] = uint32_t(i) | uint32_t(j) << 8 | uint32_t(k) << 16;
+        }
+        CK(cudaMemcpyAsync(at<uint32_t>(p, P.o_btab), btab.data(), btab.size() * 4, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(at<int>(p, P.o_bplane), boff.data(), boff.size() * 4, cudaMemcpyHostToDevice, st));
+        // level 1: bricks in sub-sweep order of the brick grid, per octant
+        std::vector<std::vector<int32_t>> goff(8), gcell(8);
+        for (int oc = 0; oc < 8; ++oc) subsweep_schedule(P.gb[0], P.gb[1], P.gb[2], oc, goff[oc], gcell[oc]);
+        const int gplanes = P.gb[0] + P.gb[1] + P.gb[2] - 2;
+        tasks.reserve(size_t(P.ntasks));
+        auto push = [&](int q, int oc, int b) {
+            int bi = b % P.gb[0], bj = (b / P.gb[0]) % P.gb[1], bk = b / (P.gb[0] * P.gb[1]);
+            tasks.push_back(make_uint2(uint32_t(q) | uint32_t(oc) << 8, uint32_t(bi) | uint32_t(bj) << 10 | uint32_t(bk) << 20));
+        };
+        if (!P.deterministic) {
+            // all problems and octants interleaved, brick sub-sweep S outermost
+            for (int S = 0; S < gplanes; ++S)
+                for (int q = 0; q < P.chunk; ++q)
+                    for (int oc = 0; oc < 8; ++oc)
+                        for (int t = goff[oc][S]; t < goff[oc][S + 1]; ++t) push(q, oc, gcell[oc][t]);
+            oct_begin[0] = 0; oct_begin[1] = int(tasks.size());
+        } else {
+            for (int oc = 0; oc < 8; ++oc) {
+                oct_begin[oc] = int(tasks.size());
+                for (int S = 0; S < gplanes; ++S)
+                    for (int q = 0; q < P.chunk; ++q)
+                        for (int t = goff[oc][S]; t < goff[oc][S + 1]; ++t) push(q, oc, gcell[oc][t]);
+            }
+            oct_begin[8] = int(tasks.size());
+        }
+        CK(cudaMemcpyAsync(at<uint2>(p, P.o_tasks), tasks.data(), tasks.size() * sizeof(uint2), cudaMemcpyHostToDevice, st));
+        CK(cudaMemsetAsync(at<unsigned>(p, P.o_flags), 0, size_t(P.chunk) * 8 * P.nbricks * 4, st));
+
+        // tensor maps over the pitched arrays (x fastest)
+        {
+            cuuint64_t d5[5] = {cuuint64_t(nx), cuuint64_t(ny), cuuint64_t(nz), cuuint64_t(NM), cuuint64_t(P.chunk)};
+            cuuint64_t s5[4] = {cuuint64_t(px) * 4, cuuint64_t(px) * ny * 4, cuuint64_t(cp) * 4, cuuint64_t(cp) * NM * 4};
+            cuuint32_t b5[5] = {cuuint32_t(P.B[0]), cuuint32_t(P.B[1]), cuuint32_t(P.B[2]), cuuint32_t(NM), 1};
+            rc = make_tensor_map(p, &SL.tmQ, at<float>(p, P.o_Q), 5, d5, s5, b5);
+            if (rc != DOCTORS_OK) return rc;
+            d5[4] = cuuint64_t(P.chunk) * G;
+            rc = make_tensor_map(p, &SL.tmPhi, at<float>(p, P.o_phiall), 5, d5, s5, b5);
+            if (rc != DOCTORS_OK) return rc;
+            rc = make_tensor_map(p, &SL.tmSig, at<float>(p, P.o_sigt), 3, d5, s5, b5);
+            if (rc != DOCTORS_OK) return rc;
+        }
+        int max_ctas = 0;
+        cudaError_t e;
+        DISPATCH_NM_FIX(NM, o.closure == 1, e = (prep_brick<NM, FIX>(P.smem, &max_ctas)));
+        if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "sweep kernel setup failed: %s (smem %zu)", cudaGetErrorString(e), P.smem);
+        if (max_ctas < 1) return fail(p, DOCTORS_CUDA, "sweep kernel does not fit an SM (smem %zu)", P.smem);
+        ctas_per_sm = o.ctas_per_sm > 0 ? std::min(o.ctas_per_sm, max_ctas) : max_ctas;
+        SL.grid = p->num_sms * ctas_per_sm;
+        SL.smem = P.smem;
+        BrickParams& bp = SL.bp;
+        bp.nx = nx; bp.ny = ny; bp.nz = nz;
+        bp.BX = P.B[0]; bp.BY = P.B[1]; bp.BZ = P.B[2];
+        bp.gbx = P.gb[0]; bp.gby = P.gb[1]; bp.gbz = P.gb[2];
+        bp.M = M; bp.g = 0; bp.Gs = G; bp.epoch = 0;
+        bp.tasks = at<uint2>(p, P.o_tasks);
+        bp.ctl = at<Control>(p, P.o_ctl);
+        bp.flags = at<unsigned>(p, P.o_flags);
+        bp.faceX = at<float>(p, P.o_fx); bp.faceY = at<float>(p, P.o_fy); bp.faceZ = at<float>(p, P.o_fz);
+        bp.Mtab = at<float>(p, P.o_mtab); bp.Dtab = at<float>(p, P.o_dtab);
+        bp.dircoef = at<float4>(p, P.o_dir); bp.leakcoef = at<float4>(p, P.o_lk);
+        bp.btab = at<uint32_t>(p, P.o_btab); bp.bplane = at<int>(p, P.o_bplane);
+        bp.state = at<ProbState>(p, P.o_state);
+        bp.leak = at<double>(p, P.o_leak);
+    } else {
+        std::vector<int32_t> cells;
+        for (int oc = 0; oc < 8; ++oc) {
+            subsweep_schedule(nx, ny, nz, oc, sched_off[oc], cells);
+            CK(cudaMemcpyAsync(at<int32_t>(p, P.o_sched) + (size_t)oc * nx * ny * nz, cells.data(), cells.size() * 4, cudaMemcpyHostToDevice, st));
+            CK(cudaStreamSynchronize(st));
+        }
+    }
+    CK(cudaStreamSynchronize(st));     // host staging vectors may go out of scope from here on
+
+    // ---- events ----
+    cudaEvent_t ev_total0, ev_total1, ev_a, ev_b;
+    CK(cudaEventCreate(&ev_total0)); CK(cudaEventCreate(&ev_total1)); CK(cudaEventCreate(&ev_a)); CK(cudaEventCreate(&ev_b));
+    std::vector<cudaEvent_t> sweep_ev;       // pairs
+    std::vector<cudaEvent_t> fixed_ev, iter_ev;
+    auto new_event = [&](std::vector<cudaEvent_t>& v) { cudaEvent_t e; cudaEventCreate(&e); v.push_back(e); return e; };
+    double ms_ray = 0.0;
+    unsigned long long sweep_launches = 0, kernel_launches = 0, updates = 0;
+    unsigned epoch = 0;
+    int* h_flag = nullptr;
+    CK(cudaMallocHost(&h_flag, 64));
+    bool not_converged = false;
+    const unsigned cblocks = unsigned((P.cells_p + 255) / 256);
+    const int red_blocks = int(std::min<long long>((P.cells_p + 255) / 256, 4LL * p->num_sms));
+
+    CK(cudaEventRecord(ev_total0, st));
+    for (int ch = 0; ch < P.nchunks; ++ch) {
+        const int prob0 = ch * P.chunk;
+        const int nq = std::min(P.chunk, P.nprob - prob0);           // problems in this chunk
+        const int src0 = P.mode == 0 ? prob0 : 0;
+        const int nsrc_c = P.mode == 0 ? nq : P.nsrc;
+        float* phi_u_c = at<float>(p, P.o_phiu) + (size_t)src0 * G * cp;
+
+        // a1: uncollided flux of the chunk's sources
+        CK(cudaEventRecord(ev_a, st));
+        k_raytrace<<<dim3(unsigned((P.cells_p + kRayThreads - 1) / kRayThreads), nsrc_c), kRayThreads, 0, st>>>(
+            md, at<uint8_t>(p, P.o_mat), at<float>(p, P.o_rho), at<SourceDev>(p, P.o_srcs), src0,
+            at<double>(p, P.o_sigt_hat), at<double>(p, P.o_spec), p->n_mat_xs, G, phi_u_c);
+        CK(cudaGetLastError());
+        ++kernel_launches;
+        CK(cudaEventRecord(ev_b, st));
+        CK(cudaEventSynchronize(ev_b));
+        { float ms = 0; cudaEventElapsedTime(&ms, ev_a, ev_b); ms_ray += ms; }
+
+        for (int g = 0; g < G; ++g) {
+            k_group_begin<<<1, 256, 0, st>>>(at<ProbState>(p, P.o_state), at<Control>(p, P.o_ctl), at<int>(p, P.o_fixediters),
+                                              prob0, nq, P.chunk, G, g, at<double>(p, P.o_bal));
+            k_sigt<<<cblocks, 256, 0, st>>>(md, at<uint8_t>(p, P.o_mat), at<float>(p, P.o_rho), at<double>(p, P.o_sigt_hat), G, g, at<float>(p, P.o_sigt));
+            cudaEvent_t f0 = new_event(fixed_ev), f1 = new_event(fixed_ev);
+            CK(cudaEventRecord(f0, st));
+            {
+                size_t sm = size_t(p->n_mat_xs) * (L + 1) * (g + 1) * 4;
+#define LAUNCH_FIXED(NMv)                                                                                          \
+    k_fixed_source<NMv><<<dim3(cblocks, nq), 256, sm, st>>>(md, at<uint8_t>(p, P.o_mat), at<float>(p, P.o_rho),       \
+        at<float>(p, P.o_sigs), p->n_mat_xs, L, G, g, at<SourceDev>(p, P.o_srcs), src0, nsrc_c, P.mode, phi_u_c,   \
+        at<float>(p, P.o_extvol), at<float>(p, P.o_phiall), at<float>(p, P.o_fixed))
+                switch (NM) { case 1: LAUNCH_FIXED(1); break; case 4: LAUNCH_FIXED(4); break; case 9: LAUNCH_FIXED(9); break; default: LAUNCH_FIXED(16); }
+#undef LAUNCH_FIXED
+            }
+            CK(cudaGetLastError());
+            CK(cudaEventRecord(f1, st));
+            kernel_launches += 3;
+
+            // fixed replay: every problem of the chunk has a count -> enqueue exactly max count, no host read
+            int max_fixed = 0; bool all_fixed = true;
+            for (int q = 0; q < nq; ++q) {
+                int f = fixed_h[(size_t)(prob0 + q) * G + g];
+                if (f <= 0) all_fixed = false;
+                max_fixed = std::max(max_fixed, f);
+            }
+            const int limit = all_fixed ? max_fixed : std::max(o.max_iters, max_fixed);
+            cudaEvent_t i0 = new_event(iter_ev), i1 = new_event(iter_ev);
+            CK(cudaEventRecord(i0, st));
+            int k = 0;
+            while (k < limit) {
+                const int batch = all_fixed ? limit : std::min(o.check_window, limit - k);
+                for (int b = 0; b < batch; ++b, ++k) {
+#define LAUNCH_UPDATE(NMv)                                                                                          \
+    k_update<NMv><<<dim3(cblocks, nq), 256, 0, st>>>(md, at<uint8_t>(p, P.o_mat), at<float>(p, P.o_rho), at<float>(p, P.o_sigs), \
+        L, G, g, G, k == 0 ? 1 : 0, at<float>(p, P.o_fixed), at<float>(p, P.o_phiall), at<float>(p, P.o_Q),          \
+        at<float>(p, P.o_phi0old), at<ProbState>(p, P.o_state), at<Control>(p, P.o_ctl), at<double>(p, P.o_leak))
+                    switch (NM) { case 1: LAUNCH_UPDATE(1); break; case 4: LAUNCH_UPDATE(4); break; case 9: LAUNCH_UPDATE(9); break; default: LAUNCH_UPDATE(16); }
+#undef LAUNCH_UPDATE
+                    ++kernel_launches;
+                    cudaEvent_t s0 = nullptr, s1 = nullptr;
+                    if (sweep_ev.size() < 16384) { s0 = new_event(sweep_ev); s1 = new_event(sweep_ev); CK(cudaEventRecord(s0, st)); }
+                    if (P.sweep_mode == 0) {
+                        SL.bp.g = g;
+                        const int nl = P.deterministic ? 8 : 1;
+                        for (int l = 0; l < nl; ++l) {
+                            SL.bp.epoch = ++epoch;
+                            SL.bp.counter_slot = l;
+                            SL.bp.task_begin = oct_begin[l];
+                            // the list is built for P.chunk problems; a short last chunk marks the missing
+                            // problems done (k_group_begin), so their tasks are skipped
+                            SL.bp.ntasks = oct_begin[l + 1] - oct_begin[l];
+                            cudaError_t e;
+                            DISPATCH_NM_FIX(NM, o.closure == 1, e = (launch_brick<NM, FIX>(SL, st)));
+                            if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "sweep launch failed: %s", cudaGetErrorString(e));
+                            ++sweep_launches; ++kernel_launches;
+                        }
+                    } else {
+                        const int planes = nx + ny + nz - 2;
+                        for (int oc = 0; oc < 8; ++oc)
+                            for (int S = 0; S < planes; ++S) {
+                                const int cnt = sched_off[oc][S + 1] - sched_off[oc][S];
+                                const int32_t* cl = at<int32_t>(p, P.o_sched) + (size_t)oc * nx * ny * nz + sched_off[oc][S];
+#define LAUNCH_SUB(NMv, FIXv)                                                                                        \
+    k_subsweep<NMv, FIXv><<<dim3((cnt + 127) / 128, nq), 128, 0, st>>>(md, cl, cnt, oc, M, at<float>(p, P.o_mtab),      \
+        at<float>(p, P.o_dtab), at<float4>(p, P.o_dir), at<float4>(p, P.o_lk), at<float>(p, P.o_sigt), at<float>(p, P.o_Q), \
+        at<float>(p, P.o_phiall), g, G, at<float>(p, P.o_ox), at<float>(p, P.o_oy), at<float>(p, P.o_oz),            \
+        at<ProbState>(p, P.o_state), at<double>(p, P.o_leak))
+                                if (o.closure == 1) { switch (NM) { case 1: LAUNCH_SUB(1, true); break; case 4: LAUNCH_SUB(4, true); break; case 9: LAUNCH_SUB(9, true); break; default: LAUNCH_SUB(16, true); } }
+                                else { switch (NM) { case 1: LAUNCH_SUB(1, false); break; case 4: LAUNCH_SUB(4, false); break; case 9: LAUNCH_SUB(9, false); break; default: LAUNCH_SUB(16, false); } }
+#undef LAUNCH_SUB
+                                ++sweep_launches; ++kernel_launches;
+                            }
+                    }
+                    if (s1) CK(cudaEventRecord(s1, st));
+                    k_check<<<dim3(red_blocks, nq), 256, 0, st>>>(md, g, G, NM, at<float>(p, P.o_phiall), at<float>(p, P.o_phi0old),
+                                                                   at<ProbState>(p, P.o_state), at<Control>(p, P.o_ctl), nq, float(o.tol), o.max_iters);
+                    ++kernel_launches;
+                }
+                CK(cudaGetLastError());
+                if (all_fixed) break;
+                CK(cudaMemcpyAsync(h_flag, &at<Control>(p, P.o_ctl)->all_done, 4, cudaMemcpyDeviceToHost, st));
+                CK(cudaStreamSynchronize(st));
+                if (*h_flag) break;
+            }
+            CK(cudaEventRecord(i1, st));
+            k_balance<<<dim3(red_blocks, nq), 256, 0, st>>>(md, g, G, NM, at<float>(p, P.o_phiall), at<float>(p, P.o_Q), at<float>(p, P.o_sigt),
+                                                             p->dx * p->dy * p->dz, at<double>(p, P.o_bal));
+            k_group_end<<<1, 256, 0, st>>>(at<ProbState>(p, P.o_state), at<double>(p, P.o_leak), at<double>(p, P.o_bal),
+                                            at<GroupResult>(p, P.o_results), prob0, nq, G, g);
+            k_keep_phi0<<<dim3(red_blocks, nq), 256, 0, st>>>(P.cells_p, g, G, NM, at<float>(p, P.o_phiall), at<float>(p, P.o_phi0all), prob0);
+            kernel_launches += 3;
+            CK(cudaGetLastError());
+        }
+        p->last_chunk_first = prob0;
+        p->last_chunk_count = nq;
+    }
+    CK(cudaEventRecord(ev_total1, st));
+    CK(cudaStreamSynchronize(st));
+    CK(cudaGetLastError());
+
+    // ---- results ----
+    std::vector<GroupResult> res(size_t(P.nprob) * G);
+    CK(cudaMemcpy(res.data(), at<GroupResult>(p, P.o_results), res.size() * sizeof(GroupResult), cudaMemcpyDeviceToHost));
+    for (size_t t = 0; t < res.size(); ++t) {
+        updates += (unsigned long long)res[t].iters * (unsigned long long)nx * ny * nz * P.ndir;
+        if (res[t].hit_max) not_converged = true;
+    }
+    if (info) {
+        for (size_t t = 0; t < res.size(); ++t) {
+            if (info->iters) info->iters[t] = res[t].iters;
+            if (info->residual) info->residual[t] = res[t].resid;
+            if (info->balance) { info->balance[3 * t] = res[t].bal_src; info->balance[3 * t + 1] = res[t].bal_col; info->balance[3 * t + 2] = res[t].leak; }
+        }
+        float ms = 0;
+        cudaEventElapsedTime(&ms, ev_total0, ev_total1); info->ms_total = ms;
+        info->ms_raytrace = ms_ray;
+        double acc = 0; for (size_t e = 0; e + 1 < sweep_ev.size(); e += 2) { cudaEventElapsedTime(&ms, sweep_ev[e], sweep_ev[e + 1]); acc += ms; }
+        info->ms_sweep = acc;
+        acc = 0; for (size_t e = 0; e + 1 < fixed_ev.size(); e += 2) { cudaEventElapsedTime(&ms, fixed_ev[e], fixed_ev[e + 1]); acc += ms; }
+        info->ms_fixed_source = acc;
+        acc = 0; for (size_t e = 0; e + 1 < iter_ev.size(); e += 2) { cudaEventElapsedTime(&ms, iter_ev[e], iter_ev[e + 1]); acc += ms; }
+        info->ms_iterate = acc;
+        info->updates = updates;
+        info->sweep_launches = sweep_launches;
+        info->kernel_launches = kernel_launches;
+        info->n_chunks = P.nchunks;
+        info->brick[0] = P.B[0]; info->brick[1] = P.B[1]; info->brick[2] = P.B[2];
+        info->ctas_per_sm = ctas_per_sm;
+    }
+    for (auto e : sweep_ev) cudaEventDestroy(e);
+    for (auto e : fixed_ev) cudaEventDestroy(e);
+    for (auto e : iter_ev) cudaEventDestroy(e);
+    cudaEventDestroy(ev_total0); cudaEventDestroy(ev_total1); cudaEventDestroy(ev_a); cudaEventDestroy(ev_b);
+    cudaFreeHost(h_flag);
+    p->solved = true;
+    if (not_converged) { p->err = "some (problem, group) stopped at max_iters"; return DOCTORS_NOT_CONVERGED; }
+    return DOCTORS_OK;
+}
+
+namespace {
+// pitched device rows -> dense rows (host or device destination)
+int copy_rows_out(doctors_problem* p, const float* src, float* out, int out_is_device, int n_fields)
+{
+    const Plan& P = p->plan;
+    cudaError_t e = cudaMemcpy2DAsync(out, size_t(p->nx) * 4, src, size_t(P.px) * 4, size_t(p->nx) * 4,
+                                      size_t(p->ny) * p->nz * n_fields, out_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, p->stream);
+    if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "copy out failed: %s", cudaGetErrorString(e));
+    e = cudaStreamSynchronize(p->stream);
+    if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "copy out failed: %s", cudaGetErrorString(e));
+    return DOCTORS_OK;
+}
+}  // namespace
+
+extern "C" int doctors_get_flux_moments(doctors_problem* p, int problem, int group, int l_max, float* out, int out_is_device)
+{
+    if (!p || !out) return DOCTORS_INVALID_ARG;
+    if (!p->solved) return fail(p, DOCTORS_BAD_STATE, "no successful solve yet");
+    const Plan& P = p->plan;
+    if (problem < 0 || problem >= P.nprob || group < 0 || group >= P.G || l_max < 0 || l_max > P.L)
+        return fail(p, DOCTORS_INVALID_ARG, "bad problem / group / l_max");
+    cudaSetDevice(p->device);
+    const size_t cp = size_t(P.cells_p);
+    if (l_max == 0) {
+        const float* src = at<float>(p, P.o_phi0all) + ((size_t)problem * P.G + group) * cp;
+        return copy_rows_out(p, src, out, out_is_device, 1);
+    }
+    if (problem < p->last_chunk_first || problem >= p->last_chunk_first + p->last_chunk_count)
+        return fail(p, DOCTORS_NOT_RETAINED, "moments l > 0 of problem %d were overwritten by a later chunk", problem);
+    const int q = problem - p->last_chunk_first;
+    const int nmo = (l_max + 1) * (l_max + 1);
+    // rows of one moment are ny*nz rows of nx; successive moments are cells_p apart = px*ny*nz -> still uniform row pitch
+    const float* src = at<float>(p, P.o_phiall) + ((size_t)q * P.G + group) * P.NM * cp;
+    return copy_rows_out(p, src, out, out_is_device, nmo);
+}
+
+extern "C" int doctors_get_uncollided_flux(doctors_problem* p, int source, int group, float* out, int out_is_device)
+{
+    if (!p || !out) return DOCTORS_INVALID_ARG;
+    if (!p->solved) return fail(p, DOCTORS_BAD_STATE, "no successful solve yet");
+    const Plan& P = p->plan;
+    if (source < 0 || source >= P.nsrc || group < 0 || group >= P.G) return fail(p, DOCTORS_INVALID_ARG, "bad source / group");
+    cudaSetDevice(p->device);
+    const float* src = at<float>(p, P.o_phiu) + ((size_t)source * P.G + group) * size_t(P.cells_p);
+    return copy_rows_out(p, src, out, out_is_device, 1);
+}

@@ -1,0 +1,171 @@
+// Shared device-side types and small PTX wrappers (sm_100a).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <cstdint>
+
+namespace doctors {
+
+constexpr int kMaxMaterials = 16;
+constexpr int kMaxMoments = 16;       // P3
+constexpr int kSweepThreads = 256;
+
+struct MeshDev {
+    int nx, ny, nz;
+    int px;                 // row pitch in cells (nx rounded up to 4: 16-byte rows for TMA)
+    long long cells_p;      // px * ny * nz
+    double dx, dy, dz;
+    double x0, y0, z0;      // centre of cell (0,0,0)
+};
+
+struct SourceDev {
+    int kind;               // 0 volume, 1 point, 2 cone
+    int vol_slot;           // kind 0: index into the volume-source array, else -1
+    double pos[3];
+    double axis[3];         // normalised
+    double cos_half;
+};
+
+// Per-problem iteration state, device resident (row a6).
+struct ProbState {
+    unsigned max_diff_bits; // max |phi0_new - phi0_old| as float bits (non-negative floats order like uints)
+    unsigned max_phi_bits;  // max |phi0_new|
+    int iters;              // sweeps done for the current group
+    int done;               // 1: this problem's current group has stopped
+    int fixed;              // > 0: stop exactly at this sweep count
+    int hit_max;            // stopped by max_iters
+    float resid;            // last delta_k
+    int pad;
+};
+
+struct Control {
+    unsigned ticket;        // last-block election of k_check
+    int all_done;           // every problem of the chunk is done for the current group
+    unsigned counters[10];  // task counters of the sweep launches of one iteration
+    unsigned pad[4];
+};
+
+// ---- small PTX wrappers ------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p)
+{
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init()
+{
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok = 0;
+    while (!ok) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok)
+            : "r"(bar), "r"(parity)
+            : "memory");
+    }
+}
+__device__ __forceinline__ void fence_proxy_async_smem()
+{
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void tma_load_5d(uint32_t dst, const CUtensorMap* map, uint32_t bar,
+                                            int c0, int c1, int c2, int c3, int c4)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes"
+        " [%0], [%1, {%3, %4, %5, %6, %7}], [%2];"
+        ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(bar),
+          "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, uint32_t bar,
+                                            int c0, int c1, int c2)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes"
+        " [%0], [%1, {%3, %4, %5}], [%2];"
+        ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(bar), "r"(c0), "r"(c1), "r"(c2)
+        : "memory");
+}
+// smem tile += into global through the TMA unit (L2 does the fp32 adds)
+__device__ __forceinline__ void tma_reduce_add_5d(const CUtensorMap* map, uint32_t src,
+                                                  int c0, int c1, int c2, int c3, int c4)
+{
+    asm volatile(
+        "cp.reduce.async.bulk.tensor.5d.global.shared::cta.add.tile.bulk_group"
+        " [%0, {%2, %3, %4, %5, %6}], [%1];"
+        ::"l"(reinterpret_cast<uint64_t>(map)), "r"(src),
+          "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4)
+        : "memory");
+}
+__device__ __forceinline__ void tma_store_5d(const CUtensorMap* map, uint32_t src,
+                                             int c0, int c1, int c2, int c3, int c4)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.5d.global.shared::cta.tile.bulk_group"
+        " [%0, {%2, %3, %4, %5, %6}], [%1];"
+        ::"l"(reinterpret_cast<uint64_t>(map)), "r"(src),
+          "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p)
+{
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_u32(unsigned* p, unsigned v)
+{
+    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+// ---- one cell, one direction: diamond difference (readings R1, R2) -----------
+//   psi = (q + cx a + cy b + cz c) / (sigt + cx + cy + cz),  out_d = 2 psi - in_d
+// FIX: any negative outflow is set to zero and the cell balance re-solved with that face's
+// diamond relation dropped (its inflow then enters with weight c_d / 2); repeat while a new
+// face flips.  Conserves the cell balance exactly.
+template <bool FIX>
+__device__ __forceinline__ float dd_cell(float q, float sig, float cx, float cy, float cz, float csum,
+                                         float a, float b, float c, float& ox, float& oy, float& oz)
+{
+    float num = fmaf(cx, a, fmaf(cy, b, fmaf(cz, c, q)));
+    float psi = __fdividef(num, sig + csum);
+    ox = fmaf(2.0f, psi, -a);
+    oy = fmaf(2.0f, psi, -b);
+    oz = fmaf(2.0f, psi, -c);
+    if (FIX) {
+        bool fx = false, fy = false, fz = false;
+#pragma unroll 1
+        for (int pass = 0; pass < 3; ++pass) {
+            bool nx_ = !fx && ox < 0.0f, ny_ = !fy && oy < 0.0f, nz_ = !fz && oz < 0.0f;
+            if (!(nx_ || ny_ || nz_)) break;
+            fx |= nx_; fy |= ny_; fz |= nz_;
+            float n2 = q, d2 = sig;
+            if (fx) n2 = fmaf(0.5f * cx, a, n2); else { n2 = fmaf(cx, a, n2); d2 += cx; }
+            if (fy) n2 = fmaf(0.5f * cy, b, n2); else { n2 = fmaf(cy, b, n2); d2 += cy; }
+            if (fz) n2 = fmaf(0.5f * cz, c, n2); else { n2 = fmaf(cz, c, n2); d2 += cz; }
+            psi = __fdividef(n2, d2);
+            ox = fx ? 0.0f : fmaf(2.0f, psi, -a);
+            oy = fy ? 0.0f : fmaf(2.0f, psi, -b);
+            oz = fz ? 0.0f : fmaf(2.0f, psi, -c);
+        }
+    }
+    return psi;
+}
+
+}  // namespace doctors
