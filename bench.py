@@ -1,0 +1,330 @@
+#!/usr/bin/env python
+"""bench.py — the driver's measurement contract for the DOCTORS hot path on B200.
+
+One "step" = one whole `doctors_solve` of the workload: ray trace (a1) -> per group fixed source
+(a2) -> source iteration {sweep of all 8 octants (a3-a5), convergence (a6)} for every source and
+group, to the 1e-5 tolerance.  Default workload = BASELINE.json configs[4] (256x256x128, 47 groups,
+P3, S8, 8 cone-beam sources batched in 2 chunks of 4) — the config the >= 50 % HBM-roofline target
+is judged on.  Metric: cell*direction*group updates per second over the whole solve.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..4] [--impl reference]
+
+N > 1 (torchrun): replicas only — the path does not shard; every rank solves the
+same workload, the time is the max over ranks, value = N * updates / time.
+`--impl reference` times the fp64 CPU oracle (as it stands) on a bounded sample of the workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "cell_direction_group_updates_per_s"
+UNIT = "updates/s"
+
+
+def rank_world():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0"))
+
+
+def measured_peak():
+    """HBM GB/s denominator: MEASURED_PEAKS.json (driver-written), else the profiling guide's fallback."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def workload_for(idx):
+    from workloads import make_config
+    wl = make_config(idx)
+    return wl
+
+
+def algorithmic_bytes_per_cell_octant(nm, batch):
+    """per (cell, octant, problem) the sweep must read Q_lm (nm*4), read-modify-write
+    phi_lm (2*nm*4) and read sigma_t (4 B shared by the `batch` problems swept together)."""
+    return nm * 4 + 2 * nm * 4 + 4.0 / batch
+
+
+# ---- clocks sampling during the timed region -----------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.tmp = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=self.tmp, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.tmp.flush()
+        self.tmp.seek(0)
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.tmp.read().splitlines():
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        try:
+            os.unlink(self.tmp.name)
+        except OSError:
+            pass
+        if sm:
+            out["sm_mhz"] = float(np.median(sm))
+            out["sm_max_mhz"] = float(max(mx))
+            out["power_w_max"] = float(max(pw))
+            out["samples"] = len(sm)
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+# ---- the oracle legs (cpu_baseline and --impl reference) -----------------------------------------
+def oracle_sample(idx):
+    """Bounded sample of config idx the oracle finishes in ~10-30 s: full mesh and quadrature,
+    first source, highest-energy group, ray trace + a fixed number of sweeps."""
+    from workloads import single_sweep_case, make_config
+    if idx <= 1:
+        wl = make_config(idx)
+        return wl, "%s: whole config (all groups, to tolerance)" % wl.name
+    sweeps = {2: 8, 3: 2, 4: 1}[idx]
+    wl = single_sweep_case(idx, groups=(0,), n_sources=1, fixed_iters=sweeps)
+    return wl, "%s mesh/quadrature, source 0, group 0 only: ray trace + %d sweep(s) of all %d directions" % (
+        wl.name, sweeps, wl.n_dir)
+
+
+def time_oracle(wl, closure):
+    from oracle import oracle
+    oracle.build()
+    cores = oracle.default_threads()
+    t0 = time.perf_counter()
+    res = oracle.solve(wl, closure=closure, threads=cores)
+    dt = time.perf_counter() - t0
+    updates = int(res["iters"].sum()) * wl.cells * wl.n_dir
+    return updates, dt, cores
+
+
+def run_reference(args):
+    rank, world, _ = rank_world()
+    if rank != 0:
+        return 0
+    wl, sample = oracle_sample(args.config)
+    full = workload_for(args.config) if args.config > 1 else wl
+    times, updates, cores = [], 0, 0
+    for i in range(args.warmup + args.steps):
+        u, dt, cores = time_oracle(wl, args.closure)
+        if i >= args.warmup:
+            times.append(dt); updates += u
+    total = sum(times)
+    v = updates / total
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * total / max(1, args.steps), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": bench_config(full, args, None),
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def bench_config(wl, args, info):
+    c = {"workload": wl.name, "mesh": [wl.nx, wl.ny, wl.nz], "groups": wl.G, "pl_order": wl.L, "sn": wl.sn,
+         "n_dir": wl.n_dir, "sources": len(wl.sources), "tol": wl.tol, "closure": args.closure,
+         "l2": "inputs larger than L2 (per-group working set > 126 MB)" if wl.cells * 33 * 4 * min(4, len(wl.sources)) > 126e6
+               else "working set fits L2; an L2 flush (256 MiB write) runs between steps",
+         "parallelism": "replicas only" if args.gpus > 1 else "1 GPU"}
+    if info is not None:
+        c.update({"source_chunks": info["n_chunks"], "brick": list(info["brick"]), "ctas_per_sm": info["ctas_per_sm"]})
+    return c
+
+
+# ---- N > 1: max over ranks ------------------------------------------------------------------------
+def aggregate_over_ranks(ms_local, updates_local, dist=None):
+    """Replicas only: time = max over ranks, updates = sum over ranks.  Works on any backend
+    (tested with gloo, world_size 2)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return ms_local, updates_local
+    import torch
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([ms_local], dtype=torch.float64, device=dev)
+    u = torch.tensor([float(updates_local)], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), int(u.item())
+
+
+def run_gpu_arm(args):
+    import torch
+    rank, world, local = rank_world()
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        torch.cuda.set_device(local)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = local if world > 1 else 0
+    torch.cuda.set_device(dev)
+    from paper_1910_11335_b200 import build
+    if rank == 0:
+        build.build()
+    if dist is not None:
+        dist.barrier()
+    import paper_1910_11335_b200 as pkg
+    pkg.load_library()                       # raises if the CUDA library is missing: no fallback
+
+    wl = workload_for(args.config)
+    nm = (wl.L + 1) ** 2
+    p = pkg.problem_from_workload(wl, device=dev)
+    kw = dict(tol=wl.tol, max_iters=wl.max_iters, closure=args.closure,
+              fixed_iters=(wl.fixed_iters if wl.fixed_iters else None))
+    if args.config == 4:
+        kw["source_chunk"] = 4               # 2 chunks of 4: all-group moments of 8 sources exceed HBM
+    flush = None
+    if wl.cells * 33 * 4 * min(4, len(wl.sources)) <= 126e6:
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+
+    def step():
+        if flush is not None:
+            flush.fill_(1)
+        return p.solve(**kw)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    sampler = ClockSampler(dev) if rank == 0 else None
+    ms_dev = ms_sweep = 0.0
+    updates = launches = sweep_launches = 0
+    t0 = time.perf_counter()
+    info = None
+    for _ in range(args.steps):
+        info = step()
+        ms_dev += info["ms_total"]; ms_sweep += info["ms_sweep"]
+        updates += info["updates"]; launches += info["kernel_launches"]; sweep_launches += info["sweep_launches"]
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    wall_ms = 1e3 * (time.perf_counter() - t0)
+    clocks = sampler.stop() if sampler else None
+    sweeps_local = int(info["iters"].sum())
+    ms_all, upd_all = aggregate_over_ranks(ms_dev, updates, dist)
+
+    # ---- e2e: host buffers in, host buffers out, through the public API, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        pin = torch.empty(wl.cells, dtype=torch.float32).pin_memory()
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        t0 = time.perf_counter()
+        p.set_mesh_materials(wl.material, wl.density, (wl.dx, wl.dy, wl.dz), wl.n_materials)
+        p.set_xs(wl.sigma_t, wl.sigma_s)
+        p.set_quadrature(wl.sn)
+        p.set_source(wl.sources, wl.mode)
+        inf2 = p.solve(**kw)
+        nprob = p.n_problems()
+        for q in range(nprob):
+            for g in range(wl.G):
+                p.get_flux_moments_into(q, g, 0, pin.data_ptr())
+        torch.cuda.synchronize()
+        e2e_s = time.perf_counter() - t0
+        e2e_ms, e2e_upd = aggregate_over_ranks(1e3 * e2e_s, inf2["updates"], dist)
+        h2d = wl.material.nbytes + wl.density.nbytes + wl.sigma_t.nbytes + wl.sigma_s.nbytes // 2 + 4096
+        h2d += sum(s.volume.nbytes for s in wl.sources if s.volume is not None)
+        e2e = {"value": e2e_upd / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(nprob * wl.G * wl.cells * 4), "steps": 1,
+               "what": "set_* from host arrays + doctors_solve + every (problem, group) scalar flux read to pinned host memory"}
+    if rank != 0:
+        p.close()
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel (k_sweep_brick) ----
+    peak, peak_src = measured_peak()
+    batch = min(4, len(wl.sources)) if wl.mode == 0 else 1
+    bytes_per = algorithmic_bytes_per_cell_octant(nm, batch)
+    problem_sweeps = updates / (wl.cells * wl.n_dir)               # sum of K[s][g] over the timed steps
+    alg_bytes = problem_sweeps * wl.cells * 8 * bytes_per
+    achieved = alg_bytes / (ms_sweep * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": "k_sweep_brick", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "peak_source": peak_src, "traffic": args.traffic,
+                "launches": int(sweep_launches), "avg_launch_ms": ms_sweep / max(1, sweep_launches),
+                "algorithmic_bytes_per_launch": alg_bytes / max(1, sweep_launches),
+                "share_of_step": ms_sweep / ms_dev,
+                "bytes_per_update": 8 * bytes_per * wl.cells / (wl.cells * wl.n_dir)}
+
+    # ---- oracle beside it (bounded sample), rank 0, N = 1 only ----
+    cpu = None
+    if world == 1 and not args.no_cpu:
+        swl, sample = oracle_sample(args.config)
+        u, dt, cores = time_oracle(swl, args.closure)
+        cpu = {"value": u / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "seconds": dt}
+
+    value = upd_all / (ms_all * 1e-3)
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_all / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic", "config": bench_config(wl, args, info),
+            "solve_ms": {"total": ms_dev / args.steps, "sweep": ms_sweep / args.steps,
+                         "raytrace": info["ms_raytrace"], "fixed_source": info["ms_fixed_source"],
+                         "iterate": info["ms_iterate"], "wall_incl_upload": wall_ms / args.steps},
+            "sweeps_per_step": sweeps_local, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+            "gpu_launches": int(launches), "clocks": clocks}
+    print(json.dumps(line), flush=True)
+    p.close()
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs index (default 4, the largest)")
+    ap.add_argument("--closure", type=int, default=1, help="0 pure diamond difference, 1 + set-to-zero fix-up (R2)")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--traffic", type=float, default=None,
+                    help="ncu dram bytes per sweep launch (from profiles/), echoed into roofline.traffic")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_gpu_arm(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

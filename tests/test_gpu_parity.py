@@ -1,0 +1,259 @@
+"""Parity of the CUDA path (through the C ABI) against the fp64 oracle — run with `-m gpu` on a B200.
+
+Bars (BASELINE.json north_star): integer schedules bit-exact; fp32 scalar flux within 1e-4 max
+relative error wherever phi > 1e-6 max(phi), per (problem, group), after the oracle's own sweep
+counts are replayed on the GPU (reading R10).  Closure per reading R2: configs 0-1 gated with both
+closures, configs 2-4 with closure 1.
+"""
+import numpy as np
+import pytest
+
+from workloads import make_config, single_sweep_case, paper_shaped
+from tests.parity_util import compare_workload, run_gpu, tiny_p3_case, masked_rel_err
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-4      # north_star: fp32 scalar flux within 1e-4 max relative error inside the mask
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1910_11335_b200 import build
+    build.build()
+    import paper_1910_11335_b200 as p
+    p.load_library()          # raises if the extension is missing: no fallback
+    return p
+
+
+# ---- a3: schedules the kernels consume, bit-exact ---------------------------------------------
+@pytest.mark.parametrize("wl_fn,brick", [(lambda: make_config(0), None), (lambda: tiny_p3_case(), None),
+                                         (lambda: tiny_p3_case(), (4, 3, 5)), (lambda: make_config(2), None)])
+def test_schedule_bit_exact(pkg, orc, wl_fn, brick):
+    wl = wl_fn()
+    p = pkg.problem_from_workload(wl)
+    for level in (0, 1, 2):
+        for octant in range(8):
+            dims, off, cells = p.debug_schedule(octant, level, brick=brick)
+            off_o, cells_o = orc.schedule(dims[0], dims[1], dims[2], octant)
+            assert np.array_equal(off, off_o) and np.array_equal(cells, cells_o), (level, octant)
+    d0, _, _ = p.debug_schedule(0, 0)
+    assert d0 == (wl.nx, wl.ny, wl.nz)
+    d1, _, _ = p.debug_schedule(0, 1, brick=brick)
+    d2, _, _ = p.debug_schedule(0, 2, brick=brick)
+    assert all(d1[a] == -(-d0[a] // d2[a]) for a in range(3))
+    p.close()
+
+
+def test_tables_match_oracle(pkg, orc):
+    wl = make_config(1)
+    p = pkg.problem_from_workload(wl)
+    om, w = p.get_quadrature()
+    om_o, w_o = orc.level_symmetric(wl.sn)
+    M, D = p.debug_tables(3)
+    Mo, Do = orc.projection_tables(3, om, w)
+    np.testing.assert_allclose(M, Mo, atol=1e-14)
+    np.testing.assert_allclose(D, Do.T, atol=1e-14)
+    np.testing.assert_allclose(np.sort(w), np.sort(w_o), atol=1e-12)
+    p.close()
+
+
+# ---- config 0 and small ragged cases: every kernel variant ------------------------------------
+@pytest.mark.parametrize("closure", [0, 1])
+@pytest.mark.parametrize("mode,det", [(0, 0), (0, 1), (1, 0)])
+def test_config0(pkg, orc, closure, mode, det):
+    wl = make_config(0)
+    ref = orc.solve(wl, closure=closure)
+    assert (ref["iters"] == 10).all()
+    worst = compare_workload(wl, ref, closure=closure, sweep_mode=mode, deterministic=det)
+    assert worst < TOL, worst
+
+
+@pytest.mark.parametrize("closure", [0, 1])
+@pytest.mark.parametrize("kind", [1, 2])
+@pytest.mark.parametrize("brick", [None, (4, 3, 5), (8, 2, 2), (12, 10, 9)])
+def test_ragged_p3(pkg, orc, closure, kind, brick):
+    """12x10x9 mesh (px padding, clipped bricks in every axis), 4 materials, P3, S8, point / cone source."""
+    wl = tiny_p3_case(kind=kind)
+    ref = orc.solve(wl, closure=closure)
+    worst = compare_workload(wl, ref, closure=closure, brick=brick)
+    assert worst < TOL, worst
+
+
+@pytest.mark.parametrize("L,sn", [(0, 4), (1, 4), (2, 6), (3, 12)])
+def test_orders(pkg, orc, L, sn):
+    wl = tiny_p3_case(nx=9, ny=7, nz=6, G=2, sn=sn, L=L, seed=11)
+    ref = orc.solve(wl, closure=1)
+    worst = compare_workload(wl, ref, closure=1)
+    assert worst < TOL, worst
+    worst = compare_workload(wl, ref, closure=1, sweep_mode=1)
+    assert worst < TOL, worst
+
+
+def test_degenerate_meshes(pkg, orc):
+    for dims in [(1, 1, 1), (1, 7, 3), (5, 1, 1), (17, 2, 1)]:
+        wl = tiny_p3_case(nx=dims[0], ny=dims[1], nz=dims[2], G=2, sn=4, L=1, seed=3)
+        ref = orc.solve(wl, closure=0)
+        worst = compare_workload(wl, ref, closure=0)
+        assert worst < TOL, (dims, worst)
+
+
+def test_higher_moments_and_balance(pkg, orc):
+    wl = tiny_p3_case()
+    ref = orc.solve(wl, closure=0)
+    p, info = run_gpu(wl, closure=0, fixed_iters=ref["iters"])
+    shape = (wl.nz, wl.ny, wl.nx)
+    for g in range(wl.G):
+        got = p.get_flux_moments(0, g, 3)
+        want = ref["phi"][0, g].reshape((16,) + shape)
+        scale = np.abs(want[0]).max()
+        assert np.abs(got - want).max() / scale < 2e-6          # all 16 moments, relative to max phi_00
+        # per-sweep particle balance of the last sweep: sum Q00 V = sum sigt phi0 V + leakage
+        src, col, leak = info["balance"][0, g]
+        assert abs(src - col - leak) < 2e-5 * src
+        np.testing.assert_allclose(info["balance"][0, g], ref["balance"][0, g], rtol=2e-5)
+    p.close()
+
+
+def test_device_convergence_matches_oracle_counts(pkg, orc):
+    """The device-side test (a6) stops within +-1 sweep of the fp64 oracle (reading R10)."""
+    wl = make_config(1)
+    ref = orc.solve(wl, closure=1)
+    p, info = run_gpu(wl, closure=1)                        # tolerance mode, no replay
+    assert info["status"] == 0
+    assert np.abs(info["iters"].astype(int) - ref["iters"]).max() <= 1
+    assert (info["residual"] < wl.tol).all()
+    got = p.get_flux_moments(0, 18, 0)[0]
+    e, _ = masked_rel_err(got, ref["phi"][0, 18, 0].reshape(got.shape))
+    assert e < 5e-4                                            # counts may differ by one sweep
+    p.close()
+
+
+def test_max_iters_reports_not_converged(pkg):
+    wl = make_config(1)
+    p = pkg.problem_from_workload(wl)
+    info = p.solve(tol=1e-12, max_iters=3, closure=1)
+    assert info["status"] == pkg.NOT_CONVERGED and (info["iters"] == 3).all()
+    p.close()
+
+
+def test_batched_sources_and_chunking(pkg, orc):
+    """Independent sources batched in one solve = each solved alone; result independent of source_chunk."""
+    wl = tiny_p3_case(kind=2)
+    s0 = wl.sources[0]
+    import copy
+    s1 = copy.deepcopy(s0); s1.pos = (0.3, 9.0, 0.2); s1.axis = (0.0, -1.0, 0.0)
+    s2 = copy.deepcopy(s0); s2.kind = 1; s2.pos = (2.0, 1.0, 8.0)
+    wl.sources = [s0, s1, s2]
+    ref = orc.solve(wl, closure=1)
+    assert ref["iters"].shape == (3, wl.G)
+    for chunk in (0, 1, 2):
+        worst = compare_workload(wl, ref, closure=1, source_chunk=chunk)
+        assert worst < TOL, (chunk, worst)
+
+
+def test_summed_sources_mode1(pkg, orc):
+    wl = tiny_p3_case(kind=2)
+    import copy
+    s1 = copy.deepcopy(wl.sources[0]); s1.pos = (0.3, 9.0, 0.2); s1.axis = (0.0, -1.0, 0.0)
+    wl.sources = [wl.sources[0], s1]
+    wl.mode = 1
+    ref = orc.solve(wl, closure=0)
+    assert ref["iters"].shape == (1, wl.G)
+    worst = compare_workload(wl, ref, closure=0)
+    assert worst < TOL, worst
+
+
+def test_api_errors(pkg):
+    wl = make_config(0)
+    p = pkg.Problem()
+    with pytest.raises(pkg.DoctorsError) as e:
+        p.set_mesh_materials(wl.material, wl.density, (1.0, -1.0, 1.0), 1)
+    assert e.value.status == pkg.INVALID_ARG
+    p.set_mesh_materials(wl.material, wl.density, (1.0, 1.0, 1.0), 1)
+    up = np.zeros((1, 1, 2, 2)); up[0, 0, 1, 0] = 0.1                      # upscatter entry
+    with pytest.raises(pkg.DoctorsError):
+        p.set_xs(np.full((1, 2), 0.2), up)
+    p.set_xs(wl.sigma_t, wl.sigma_s)
+    with pytest.raises(pkg.DoctorsError):
+        p.set_quadrature(10)
+    with pytest.raises(pkg.DoctorsError) as e:
+        p.workspace_bytes()                                                # quadrature / source missing
+    assert e.value.status == pkg.BAD_STATE
+    p.set_quadrature(2)
+    p.set_source(wl.sources, 0)
+    L = pkg.load_library()
+    import ctypes
+    buf = np.zeros(wl.cells, dtype=np.float32)
+    assert L.doctors_get_flux_moments(p._h, 0, 0, 0, ctypes.c_void_p(buf.ctypes.data), 0) == pkg.BAD_STATE
+    p.solve(fixed_iters=2)
+    with pytest.raises(pkg.DoctorsError):
+        p.get_flux_moments(0, 1, 0)
+    p.close()
+
+
+# ---- the BASELINE configs -----------------------------------------------------------------------
+@pytest.mark.parametrize("closure", [0, 1])
+def test_config1_full(pkg, orc, closure):
+    wl = make_config(1)
+    ref = orc.solve(wl, closure=closure)
+    worst = compare_workload(wl, ref, closure=closure)
+    assert worst < TOL, worst
+
+
+def test_config2_full_closure1(pkg, orc):
+    wl = make_config(2)
+    ref = orc.solve(wl, closure=1)
+    worst = compare_workload(wl, ref, closure=1)
+    assert worst < TOL, worst
+    assert ref["phi"][:, :, 0].min() >= 0.0
+
+
+def test_config3_full_mesh_sampled_groups(pkg, orc):
+    """128x128x64, S16 (36 directions per octant), P3: full mesh and quadrature, groups {0, 18}, 3 sweeps."""
+    wl = single_sweep_case(3, groups=(0, 18), fixed_iters=3)
+    ref = orc.solve(wl, closure=1)
+    worst = compare_workload(wl, ref, closure=1)
+    assert worst < TOL, worst
+
+
+def test_config4_full_mesh_one_source(pkg, orc):
+    """256x256x128 GRF phantom in the bench's launch configuration: one source, the lowest-energy
+    group pair, 2 sweeps each, against the oracle on every cell."""
+    wl = single_sweep_case(4, groups=(45, 46), n_sources=1, fixed_iters=2)
+    ref = orc.solve(wl, closure=1)
+    worst = compare_workload(wl, ref, closure=1)
+    assert worst < TOL, worst
+
+
+def test_config4_batched_properties(pkg):
+    """Properties that hold at any size, on the batched 4-source launch the bench times: exact
+    per-sweep particle balance, non-negative flux under closure 1, and the rotational symmetry
+    that maps source s to s+2 is NOT assumed (random phantom) — instead each problem of the
+    batch must equal the same problem solved alone."""
+    wl = single_sweep_case(4, groups=(0, 20, 46), n_sources=4, fixed_iters=3)
+    p, info = run_gpu(wl, closure=1, fixed_iters=3)
+    assert info["brick"] == (8, 8, 8) or info["brick"][0] % 4 == 0
+    for q in range(4):
+        for g in range(3):
+            src, col, leak = info["balance"][q, g]
+            assert src > 0 and abs(src - col - leak) < 5e-5 * src, (q, g, src, col, leak)
+    batch = [p.get_flux_moments(q, 2, 0)[0].copy() for q in range(4)]
+    assert min(b.min() for b in batch) >= 0.0
+    p.close()
+    import copy
+    w1 = copy.copy(wl)
+    w1.sources = [wl.sources[2]]
+    p1, _ = run_gpu(w1, closure=1, fixed_iters=3)
+    alone = p1.get_flux_moments(0, 2, 0)[0]
+    e, n = masked_rel_err(batch[2], alone)
+    assert n > 1000 and e < 2e-5, e                           # fp32 summation order (L2 reduce-add) only
+    p1.close()
+
+
+def test_paper_shaped_ct_summed(pkg, orc):
+    """Row f1: the paper's coarse CT workload shape (64x64x16, S6 P0, 16 cone beams summed), 6 groups."""
+    wl = paper_shaped(ct=True, G=6)
+    ref = orc.solve(wl, closure=1)
+    worst = compare_workload(wl, ref, closure=1)
+    assert worst < TOL, worst
