@@ -38,12 +38,13 @@ struct Plan {
     int G = 0, L = 0, NM = 0, ndir = 0, M = 0;
     int mode = 0, sweep_mode = 0, deterministic = 0;
     int B[3] = {0, 0, 0}, gb[3] = {0, 0, 0};
+    int W = 1;                      // sweep warps per CTA
     long long nbricks = 0, ntasks = 0;
     size_t smem = 0;
     // offsets
-    size_t o_mat, o_rho, o_sigt_hat, o_sigs, o_spec, o_srcs, o_extvol, o_mtab, o_dtab, o_dir, o_lk,
+    size_t o_mat, o_rho, o_sigt_hat, o_sigs, o_spec, o_srcs, o_extvol, o_mtab, o_dtab, o_lk,
         o_sigt, o_Q, o_fixed, o_phi0old, o_phiall, o_phi0all, o_phiu, o_state, o_ctl, o_leak, o_bal,
-        o_results, o_fixediters, o_tasks, o_flags, o_fx, o_fy, o_fz, o_btab, o_bplane, o_sched, o_ox, o_oy, o_oz;
+        o_results, o_fixediters, o_tasks, o_flags, o_fx, o_fy, o_fz, o_dird, o_dbg, o_sched, o_ox, o_oy, o_oz;
     size_t face_x_n = 0, face_y_n = 0, face_z_n = 0;
     size_t total = 0;
 };
@@ -104,15 +105,15 @@ int nprob_of(const doctors_problem* p) { return p->mode == 0 ? int(p->sources.si
 void auto_brick(int NM, int M, int nx, int ny, int nz, const int* req, int B[3])
 {
     if (req && req[0] > 0 && req[1] > 0 && req[2] > 0) { B[0] = req[0]; B[1] = req[1]; B[2] = req[2]; return; }
-    const int cand[4][3] = {{8, 8, 8}, {8, 8, 4}, {8, 4, 4}, {4, 4, 4}};
+    // cross section = the 32 lanes of a warp (8 x 4, reshaped for thin meshes); BX as long as shared memory allows
+    B[1] = std::min(8, ny);
+    B[2] = std::min(32 / B[1], nz);
+    if (B[2] < 4 && B[1] < ny) B[1] = std::min(32 / B[2], ny);
+    const int cand[4] = {16, 12, 8, 4};
     for (int c = 0; c < 4; ++c) {
-        B[0] = cand[c][0]; B[1] = cand[c][1]; B[2] = cand[c][2];
-        if (brick_smem_layout(NM, B[0], B[1], B[2], M).total <= 75 * 1024) break;
+        B[0] = std::min(cand[c], (nx + 3) / 4 * 4);
+        if (brick_smem_layout(NM, B[0], B[1], B[2], M).total <= 74 * 1024) break;
     }
-    // do not make bricks larger than the mesh needs
-    B[0] = std::min(B[0], (nx + 3) / 4 * 4);
-    B[1] = std::min(B[1], ny);
-    B[2] = std::min(B[2], nz);
 }
 
 // Lay out the workspace.  chunk = problems solved together.
@@ -138,6 +139,7 @@ Plan make_plan(const doctors_problem* p, const doctors_solve_opts* o, int chunk)
     P.nbricks = (long long)P.gb[0] * P.gb[1] * P.gb[2];
     P.ntasks = P.nbricks * 8 * P.chunk;
     P.smem = brick_smem_layout(P.NM, P.B[0], P.B[1], P.B[2], P.M).total;
+    { int dpw = (P.M + kMaxSweepWarps - 1) / kMaxSweepWarps; P.W = (P.M + dpw - 1) / dpw; }
 
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t r = off; off = align_up(off + bytes, 256); return r; };
@@ -154,9 +156,9 @@ Plan make_plan(const doctors_problem* p, const doctors_solve_opts* o, int chunk)
     P.o_extvol = take(size_t(P.nvol) * G * cp * 4);
     P.o_mtab = take(size_t(P.ndir) * nm * 4);
     P.o_dtab = take(size_t(P.ndir) * nm * 4);
-    P.o_dir = take(size_t(P.ndir) * 16);
     P.o_lk = take(size_t(P.ndir) * 16);
-    P.o_sigt = take(cp * 4);
+    P.o_dird = take(size_t(P.ndir) * 32);
+    P.o_sigt = take(cp * 8);
     P.o_Q = take(size_t(P.chunk) * nm * cp * 4);
     P.o_fixed = take(size_t(P.chunk) * nm * cp * 4);
     P.o_phi0old = take(size_t(P.chunk) * cp * 4);
@@ -175,18 +177,17 @@ Plan make_plan(const doctors_problem* p, const doctors_solve_opts* o, int chunk)
         P.face_z_n = size_t(P.M) * P.B[0] * P.B[1];
         P.o_tasks = take(size_t(P.ntasks) * sizeof(uint2));
         P.o_flags = take(size_t(P.chunk) * 8 * P.nbricks * 4);
-        P.o_fx = take(size_t(P.chunk) * 8 * P.gb[1] * P.gb[2] * P.face_x_n * 4);
-        P.o_fy = take(size_t(P.chunk) * 8 * P.gb[0] * P.gb[2] * P.face_y_n * 4);
-        P.o_fz = take(size_t(P.chunk) * 8 * P.gb[0] * P.gb[1] * P.face_z_n * 4);
-        P.o_btab = take(size_t(P.B[0]) * P.B[1] * P.B[2] * 4);
-        P.o_bplane = take(size_t(P.B[0] + P.B[1] + P.B[2]) * 4);
+        P.o_fx = take(size_t(P.chunk) * 8 * P.gb[1] * P.gb[2] * P.face_x_n * 8);
+        P.o_fy = take(size_t(P.chunk) * 8 * P.gb[0] * P.gb[2] * P.face_y_n * 8);
+        P.o_fz = take(size_t(P.chunk) * 8 * P.gb[0] * P.gb[1] * P.face_z_n * 8);
+        P.o_dbg = take(size_t(P.B[0]) * P.B[1] * P.B[2] * 4);
         P.o_sched = P.o_ox = P.o_oy = P.o_oz = 0;
     } else {
         P.o_sched = take(size_t(8) * p->nx * p->ny * p->nz * 4);
-        P.o_ox = take(size_t(P.chunk) * P.M * cp * 4);
-        P.o_oy = take(size_t(P.chunk) * P.M * cp * 4);
-        P.o_oz = take(size_t(P.chunk) * P.M * cp * 4);
-        P.o_tasks = P.o_flags = P.o_fx = P.o_fy = P.o_fz = P.o_btab = P.o_bplane = 0;
+        P.o_ox = take(size_t(P.chunk) * P.M * cp * 8);
+        P.o_oy = take(size_t(P.chunk) * P.M * cp * 8);
+        P.o_oz = take(size_t(P.chunk) * P.M * cp * 8);
+        P.o_tasks = P.o_flags = P.o_fx = P.o_fy = P.o_fz = P.o_dbg = 0;
     }
     P.total = off;
     P.ok = true;
@@ -555,10 +556,11 @@ template <typename T>
 T* at(doctors_problem* p, size_t off) { return reinterpret_cast<T*>(static_cast<char*>(p->ws) + off); }
 
 int make_tensor_map(doctors_problem* p, CUtensorMap* tm, void* base, int rank, const cuuint64_t* dims,
-                    const cuuint64_t* strides_bytes /*rank-1*/, const cuuint32_t* box)
+                    const cuuint64_t* strides_bytes /*rank-1*/, const cuuint32_t* box,
+                    CUtensorMapDataType dtype = CU_TENSOR_MAP_DATA_TYPE_FLOAT32)
 {
     cuuint32_t es[5] = {1, 1, 1, 1, 1};
-    CUresult r = p->encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, cuuint32_t(rank), base, dims, strides_bytes, box, es,
+    CUresult r = p->encode(tm, dtype, cuuint32_t(rank), base, dims, strides_bytes, box, es,
                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                            CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(p, DOCTORS_CUDA, "cuTensorMapEncodeTiled failed (%d)", int(r));
@@ -575,16 +577,16 @@ struct SweepLaunch {
 template <int NM, bool FIX>
 cudaError_t launch_brick(const SweepLaunch& S, cudaStream_t st)
 {
-    k_sweep_brick<NM, FIX><<<S.grid, kSweepThreads, S.smem, st>>>(S.tmQ, S.tmPhi, S.tmSig, S.bp);
+    k_sweep_brick<NM, FIX><<<S.grid, 32 * S.bp.W, S.smem, st>>>(S.tmQ, S.tmPhi, S.tmSig, S.bp);
     return cudaGetLastError();
 }
 
 template <int NM, bool FIX>
-cudaError_t prep_brick(size_t smem, int* max_ctas)
+cudaError_t prep_brick(size_t smem, int threads, int* max_ctas)
 {
     cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<NM, FIX>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(max_ctas, k_sweep_brick<NM, FIX>, kSweepThreads, smem);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(max_ctas, k_sweep_brick<NM, FIX>, threads, smem);
 }
 
 #define DISPATCH_NM_FIX(NMv, FIXv, EXPR)                                         \
@@ -621,8 +623,8 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
     if (o.check_window <= 0) o.check_window = 12;
     if (o.closure != 0 && o.closure != 1) return fail(p, DOCTORS_INVALID_ARG, "closure must be 0 or 1");
     if (o.sweep_mode != 0 && o.sweep_mode != 1) return fail(p, DOCTORS_INVALID_ARG, "sweep_mode must be 0 or 1");
-    if (o.brick[0] > 0 && (o.brick[0] % 4 != 0 || o.brick[0] > 64 || o.brick[1] > 64 || o.brick[2] > 64 || o.brick[1] <= 0 || o.brick[2] <= 0))
-        return fail(p, DOCTORS_INVALID_ARG, "brick extents must be 1..64 with brick[0] a multiple of 4");
+    if (o.brick[0] > 0 && (o.brick[0] % 4 != 0 || o.brick[0] > 64 || o.brick[1] <= 0 || o.brick[2] <= 0 || o.brick[1] * o.brick[2] > 32))
+        return fail(p, DOCTORS_INVALID_ARG, "brick: brick[0] a multiple of 4 (<= 64), brick[1] * brick[2] <= 32 (the lanes of a warp)");
     if (!p->ws) return fail(p, DOCTORS_ALLOC, "no workspace set");
     CK(cudaSetDevice(p->device));
     cudaStream_t st = p->stream;
@@ -687,10 +689,11 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
     std::vector<double> Mt, Dt;
     projection_tables(L, p->omega, p->w, Mt, Dt);
     std::vector<float> Mt_f(Mt.begin(), Mt.end()), Dt_f(Dt.begin(), Dt.end());
-    std::vector<float4> dirc(P.ndir), lkc(P.ndir);
+    std::vector<float4> lkc(P.ndir);
+    std::vector<double> dird(size_t(P.ndir) * 4);
     for (int n = 0; n < P.ndir; ++n) {
         double cx = 2.0 * std::fabs(p->omega[3 * n]) / p->dx, cy = 2.0 * std::fabs(p->omega[3 * n + 1]) / p->dy, cz = 2.0 * std::fabs(p->omega[3 * n + 2]) / p->dz;
-        dirc[n] = make_float4(float(cx), float(cy), float(cz), float(cx + cy + cz));
+        dird[4 * n] = cx; dird[4 * n + 1] = cy; dird[4 * n + 2] = cz; dird[4 * n + 3] = cx + cy + cz;
         lkc[n] = make_float4(float(p->w[n] * std::fabs(p->omega[3 * n]) * p->dy * p->dz),
                              float(p->w[n] * std::fabs(p->omega[3 * n + 1]) * p->dx * p->dz),
                              float(p->w[n] * std::fabs(p->omega[3 * n + 2]) * p->dx * p->dy), 0.0f);
@@ -703,7 +706,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
     CK(cudaMemcpyAsync(at<SourceDev>(p, P.o_srcs), sdev.data(), sdev.size() * sizeof(SourceDev), cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(at<float>(p, P.o_mtab), Mt_f.data(), Mt_f.size() * 4, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(at<float>(p, P.o_dtab), Dt_f.data(), Dt_f.size() * 4, cudaMemcpyHostToDevice, st));
-    CK(cudaMemcpyAsync(at<float4>(p, P.o_dir), dirc.data(), dirc.size() * 16, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(at<double>(p, P.o_dird), dird.data(), dird.size() * 8, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(at<float4>(p, P.o_lk), lkc.data(), lkc.size() * 16, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(at<int>(p, P.o_fixediters), fixed_h.data(), fixed_h.size() * 4, cudaMemcpyHostToDevice, st));
 
@@ -714,17 +717,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
     SweepLaunch SL;
     int ctas_per_sm = 0;
     if (P.sweep_mode == 0) {
-        // level 2: cells of a full brick, sweep-space order (octant 0); the kernel mirrors per octant
-        std::vector<int32_t> boff, bcell;
-        subsweep_schedule(P.B[0], P.B[1], P.B[2], 0, boff, bcell);
-        std::vector<uint32_t> btab(bcell.size());
-        for (size_t t = 0; t < bcell.size(); ++t) {
-            int c = bcell[t];
-            int i = c % P.B[0], j = (c / P.B[0]) % P.B[1], k = c / (P.B[0] * P.B[1]);
-            btab[t] = uint32_t(i) | uint32_t(j) << 8 | uint32_t(k) << 16;
-        }
-        CK(cudaMemcpyAsync(at<uint32_t>(p, P.o_btab), btab.data(), btab.size() * 4, cudaMemcpyHostToDevice, st));
-        CK(cudaMemcpyAsync(at<int>(p, P.o_bplane), boff.data(), boff.size() * 4, cudaMemcpyHostToDevice, st));
+        // level 2 (cells of a brick) needs no table: lane (j',k') at step s updates i' = s - j' - k' (Eq. 8)
         // level 1: bricks in sub-sweep order of the brick grid, per octant
         std::vector<std::vector<int32_t>> goff(8), gcell(8);
         for (int oc = 0; oc < 8; ++oc) subsweep_schedule(P.gb[0], P.gb[1], P.gb[2], oc, goff[oc], gcell[oc]);
@@ -763,12 +756,13 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
             d5[4] = cuuint64_t(P.chunk) * G;
             rc = make_tensor_map(p, &SL.tmPhi, at<float>(p, P.o_phiall), 5, d5, s5, b5);
             if (rc != DOCTORS_OK) return rc;
-            rc = make_tensor_map(p, &SL.tmSig, at<float>(p, P.o_sigt), 3, d5, s5, b5);
+            cuuint64_t s3[2] = {cuuint64_t(px) * 8, cuuint64_t(px) * ny * 8};
+            rc = make_tensor_map(p, &SL.tmSig, at<double>(p, P.o_sigt), 3, d5, s3, b5, CU_TENSOR_MAP_DATA_TYPE_FLOAT64);
             if (rc != DOCTORS_OK) return rc;
         }
         int max_ctas = 0;
         cudaError_t e;
-        DISPATCH_NM_FIX(NM, o.closure == 1, e = (prep_brick<NM, FIX>(P.smem, &max_ctas)));
+        DISPATCH_NM_FIX(NM, o.closure == 1, e = (prep_brick<NM, FIX>(P.smem, 32 * P.W, &max_ctas)));
         if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "sweep kernel setup failed: %s (smem %zu)", cudaGetErrorString(e), P.smem);
         if (max_ctas < 1) return fail(p, DOCTORS_CUDA, "sweep kernel does not fit an SM (smem %zu)", P.smem);
         ctas_per_sm = o.ctas_per_sm > 0 ? std::min(o.ctas_per_sm, max_ctas) : max_ctas;
@@ -778,14 +772,14 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         bp.nx = nx; bp.ny = ny; bp.nz = nz;
         bp.BX = P.B[0]; bp.BY = P.B[1]; bp.BZ = P.B[2];
         bp.gbx = P.gb[0]; bp.gby = P.gb[1]; bp.gbz = P.gb[2];
-        bp.M = M; bp.g = 0; bp.Gs = G; bp.epoch = 0;
+        bp.M = M; bp.W = P.W; bp.g = 0; bp.Gs = G; bp.epoch = 0;
         bp.tasks = at<uint2>(p, P.o_tasks);
         bp.ctl = at<Control>(p, P.o_ctl);
         bp.flags = at<unsigned>(p, P.o_flags);
-        bp.faceX = at<float>(p, P.o_fx); bp.faceY = at<float>(p, P.o_fy); bp.faceZ = at<float>(p, P.o_fz);
+        bp.faceX = at<double>(p, P.o_fx); bp.faceY = at<double>(p, P.o_fy); bp.faceZ = at<double>(p, P.o_fz);
         bp.Mtab = at<float>(p, P.o_mtab); bp.Dtab = at<float>(p, P.o_dtab);
-        bp.dircoef = at<float4>(p, P.o_dir); bp.leakcoef = at<float4>(p, P.o_lk);
-        bp.btab = at<uint32_t>(p, P.o_btab); bp.bplane = at<int>(p, P.o_bplane);
+        bp.dird = at<double>(p, P.o_dird); bp.leakcoef = at<float4>(p, P.o_lk);
+        bp.dbg_plane = nullptr;
         bp.state = at<ProbState>(p, P.o_state);
         bp.leak = at<double>(p, P.o_leak);
     } else {
@@ -835,7 +829,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         for (int g = 0; g < G; ++g) {
             k_group_begin<<<1, 256, 0, st>>>(at<ProbState>(p, P.o_state), at<Control>(p, P.o_ctl), at<int>(p, P.o_fixediters),
                                               prob0, nq, P.chunk, G, g, at<double>(p, P.o_bal));
-            k_sigt<<<cblocks, 256, 0, st>>>(md, at<uint8_t>(p, P.o_mat), at<float>(p, P.o_rho), at<double>(p, P.o_sigt_hat), G, g, at<float>(p, P.o_sigt));
+            k_sigt<<<cblocks, 256, 0, st>>>(md, at<uint8_t>(p, P.o_mat), at<float>(p, P.o_rho), at<double>(p, P.o_sigt_hat), G, g, at<double>(p, P.o_sigt));
             cudaEvent_t f0 = new_event(fixed_ev), f1 = new_event(fixed_ev);
             CK(cudaEventRecord(f0, st));
             {
@@ -897,8 +891,8 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
                                 const int32_t* cl = at<int32_t>(p, P.o_sched) + (size_t)oc * nx * ny * nz + sched_off[oc][S];
 #define LAUNCH_SUB(NMv, FIXv)                                                                                        \
     k_subsweep<NMv, FIXv><<<dim3((cnt + 127) / 128, nq), 128, 0, st>>>(md, cl, cnt, oc, M, at<float>(p, P.o_mtab),      \
-        at<float>(p, P.o_dtab), at<float4>(p, P.o_dir), at<float4>(p, P.o_lk), at<float>(p, P.o_sigt), at<float>(p, P.o_Q), \
-        at<float>(p, P.o_phiall), g, G, at<float>(p, P.o_ox), at<float>(p, P.o_oy), at<float>(p, P.o_oz),            \
+        at<float>(p, P.o_dtab), at<double>(p, P.o_dird), at<float4>(p, P.o_lk), at<double>(p, P.o_sigt), at<float>(p, P.o_Q), \
+        at<float>(p, P.o_phiall), g, G, at<double>(p, P.o_ox), at<double>(p, P.o_oy), at<double>(p, P.o_oz),            \
         at<ProbState>(p, P.o_state), at<double>(p, P.o_leak))
                                 if (o.closure == 1) { switch (NM) { case 1: LAUNCH_SUB(1, true); break; case 4: LAUNCH_SUB(4, true); break; case 9: LAUNCH_SUB(9, true); break; default: LAUNCH_SUB(16, true); } }
                                 else { switch (NM) { case 1: LAUNCH_SUB(1, false); break; case 4: LAUNCH_SUB(4, false); break; case 9: LAUNCH_SUB(9, false); break; default: LAUNCH_SUB(16, false); } }
@@ -918,7 +912,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
                 if (*h_flag) break;
             }
             CK(cudaEventRecord(i1, st));
-            k_balance<<<dim3(red_blocks, nq), 256, 0, st>>>(md, g, G, NM, at<float>(p, P.o_phiall), at<float>(p, P.o_Q), at<float>(p, P.o_sigt),
+            k_balance<<<dim3(red_blocks, nq), 256, 0, st>>>(md, g, G, NM, at<float>(p, P.o_phiall), at<float>(p, P.o_Q), at<double>(p, P.o_sigt),
                                                              p->dx * p->dy * p->dz, at<double>(p, P.o_bal));
             k_group_end<<<1, 256, 0, st>>>(at<ProbState>(p, P.o_state), at<double>(p, P.o_leak), at<double>(p, P.o_bal),
                                             at<GroupResult>(p, P.o_results), prob0, nq, G, g);

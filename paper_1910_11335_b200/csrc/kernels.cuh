@@ -91,14 +91,15 @@ k_raytrace(MeshDev m, const uint8_t* __restrict__ mat, const float* __restrict__
     }
 }
 
-// sigma_t(c) = density(c) * sigt_hat[material(c)][g] for the current group (fp32 for the sweep).
+// sigma_t(c) = density(c) * sigt_hat[material(c)][g] for the current group, kept in fp64: the face
+// recurrence of the sweep is sensitive to the rounding of sigma_t (device_common.cuh, dd_cell).
 __global__ void k_sigt(MeshDev m, const uint8_t* __restrict__ mat, const float* __restrict__ rho,
-                       const double* __restrict__ sigt_hat, int G, int g, float* __restrict__ sigt)
+                       const double* __restrict__ sigt_hat, int G, int g, double* __restrict__ sigt)
 {
     long long cp = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (cp >= m.cells_p) return;
     int i = int(cp % m.px);
-    sigt[cp] = i < m.nx ? float((double)rho[cp] * sigt_hat[mat[cp] * G + g]) : 0.0f;
+    sigt[cp] = i < m.nx ? (double)rho[cp] * sigt_hat[mat[cp] * G + g] : 0.0;
 }
 
 // Real harmonics of reading R4 in Cartesian form (fp32), l <= 3.
@@ -323,7 +324,7 @@ k_check(MeshDev m, int g, int Gs, int NM, const float* __restrict__ phi, const f
 // Balance terms of the last sweep of a group (SURVEY pins): sum Q_00 V and sum sigma_t phi_00 V, fp64.
 __global__ void __launch_bounds__(256)
 k_balance(MeshDev m, int g, int Gs, int NM, const float* __restrict__ phi, const float* __restrict__ Q,
-          const float* __restrict__ sigt, double V, double* out /*[prob][2]*/)
+          const double* __restrict__ sigt, double V, double* out /*[prob][2]*/)
 {
     const int p = blockIdx.y;
     const float* ph = phi + ((size_t)p * Gs + g) * NM * m.cells_p;
@@ -332,7 +333,7 @@ k_balance(MeshDev m, int g, int Gs, int NM, const float* __restrict__ phi, const
     for (long long cp = (long long)blockIdx.x * blockDim.x + threadIdx.x; cp < m.cells_p;
          cp += (long long)gridDim.x * blockDim.x) {
         sq += (double)q[cp];
-        sc += (double)sigt[cp] * (double)ph[cp];
+        sc += sigt[cp] * (double)ph[cp];
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -350,15 +351,15 @@ k_balance(MeshDev m, int g, int Gs, int NM, const float* __restrict__ phi, const
 // of one octant; thread t handles voxel cell_of[plane_offset[S] + t] (Eq. 8, Table 1 order).
 // Unlike the paper, the directions of the octant are looped inside the thread, so the voxel's
 // moments are reduced in registers and written once (no race on the voxel's fluence).
-// Face fluxes of the octant live in global arrays out_d [prob][M][cells_p].
+// Face fluxes of the octant live in global fp64 arrays out_d [prob][M][cells_p].
 // =========================================================================================
 template <int NM, bool FIX>
 __global__ void __launch_bounds__(128)
 k_subsweep(MeshDev m, const int32_t* __restrict__ cells, int count, int octant, int M,
-           const float* __restrict__ Mtab, const float* __restrict__ Dtab, const float4* __restrict__ dircoef,
+           const float* __restrict__ Mtab, const float* __restrict__ Dtab, const double* __restrict__ dird,
            const float4* __restrict__ leakcoef,
-           const float* __restrict__ sigt, const float* __restrict__ Q, float* __restrict__ phi, int g, int Gs,
-           float* __restrict__ outx, float* __restrict__ outy, float* __restrict__ outz,
+           const double* __restrict__ sigt, const float* __restrict__ Q, float* __restrict__ phi, int g, int Gs,
+           double* __restrict__ outx, double* __restrict__ outy, double* __restrict__ outz,
            const ProbState* __restrict__ st, double* leak)
 {
     const int p = blockIdx.y;
@@ -376,7 +377,7 @@ k_subsweep(MeshDev m, const int32_t* __restrict__ cells, int count, int octant, 
         const size_t cux = (size_t)iu + (size_t)m.px * (j + (size_t)m.ny * k);
         const size_t cuy = (size_t)i + (size_t)m.px * (ju + (size_t)m.ny * k);
         const size_t cuz = (size_t)i + (size_t)m.px * (j + (size_t)m.ny * ku);
-        const float sg = sigt[cp];
+        const double sg = sigt[cp];
         float q[NM], acc[NM];
         const float* qp = Q + (size_t)p * NM * m.cells_p + cp;
 #pragma unroll
@@ -386,18 +387,18 @@ k_subsweep(MeshDev m, const int32_t* __restrict__ cells, int count, int octant, 
             float qn = 0.0f;
 #pragma unroll
             for (int lm = 0; lm < NM; ++lm) qn = fmaf(Mtab[nd * NM + lm], q[lm], qn);
-            const float4 dc = dircoef[nd];
+            const double dcx = dird[4 * nd], dcy = dird[4 * nd + 1], dcz = dird[4 * nd + 2], dcs = dird[4 * nd + 3];
             const size_t fo = ((size_t)p * M + n) * m.cells_p;
-            float a = hx ? outx[fo + cux] : 0.0f;          // vacuum inflow on the boundary
-            float b = hy ? outy[fo + cuy] : 0.0f;
-            float cz = hz ? outz[fo + cuz] : 0.0f;
-            float ox, oy, oz;
-            float psi = dd_cell<FIX>(qn, sg, dc.x, dc.y, dc.z, dc.w, a, b, cz, ox, oy, oz);
+            double a = hx ? outx[fo + cux] : 0.0;          // vacuum inflow on the boundary
+            double b = hy ? outy[fo + cuy] : 0.0;
+            double cz = hz ? outz[fo + cuz] : 0.0;
+            double ox, oy, oz;
+            float psi = dd_cell<FIX>(qn, sg, dcx, dcy, dcz, dcs, a, b, cz, ox, oy, oz);
             outx[fo + cp] = ox; outy[fo + cp] = oy; outz[fo + cp] = oz;
             const float4 lc = leakcoef[nd];
-            if (bx) lk = fmaf(lc.x, ox, lk);
-            if (by) lk = fmaf(lc.y, oy, lk);
-            if (bz) lk = fmaf(lc.z, oz, lk);
+            if (bx) lk = fmaf(lc.x, (float)ox, lk);
+            if (by) lk = fmaf(lc.y, (float)oy, lk);
+            if (bz) lk = fmaf(lc.z, (float)oz, lk);
 #pragma unroll
             for (int lm = 0; lm < NM; ++lm) acc[lm] = fmaf(Dtab[nd * NM + lm], psi, acc[lm]);
         }
