@@ -34,6 +34,7 @@ def build(force=False, verbose=False):
            "-o", LIB] + [os.path.join(CSRC, f) for f in SOURCES]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
+    cmd[1:1] = os.environ.get("DOCTORS_NVCC_FLAGS", "").split()
     subprocess.check_call(cmd)
     return LIB
 

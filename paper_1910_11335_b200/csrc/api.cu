@@ -780,6 +780,10 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         bp.Mtab = at<float>(p, P.o_mtab); bp.Dtab = at<float>(p, P.o_dtab);
         bp.dird = at<double>(p, P.o_dird); bp.leakcoef = at<float4>(p, P.o_lk);
         bp.dbg_plane = nullptr;
+        bp.dbg_time = nullptr;
+#ifdef DOCTORS_TIMING
+        { static long long* dt = nullptr; if (!dt) { cudaMalloc(&dt, 16 * 8); } cudaMemset(dt, 0, 16 * 8); bp.dbg_time = dt; }
+#endif
         bp.state = at<ProbState>(p, P.o_state);
         bp.leak = at<double>(p, P.o_leak);
     } else {
@@ -927,6 +931,15 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
     CK(cudaStreamSynchronize(st));
     CK(cudaGetLastError());
 
+#ifdef DOCTORS_TIMING
+    if (P.sweep_mode == 0 && SL.bp.dbg_time) {
+        long long h[16];
+        cudaMemcpy(h, SL.bp.dbg_time, sizeof h, cudaMemcpyDeviceToHost);
+        const char* nm[9] = {"fetch", "dep-wait", "face-load", "tma-wait", "phase0", "wavefront", "face-store+release", "phase2", "tail"};
+        double tot = 0; for (int i = 0; i < 9; ++i) tot += double(h[i]);
+        for (int i = 0; i < 9; ++i) fprintf(stderr, "  [timing] %-20s %6.2f %%  %.3e cycles\n", nm[i], 100.0 * h[i] / tot, double(h[i]));
+    }
+#endif
     // ---- results ----
     std::vector<GroupResult> res(size_t(P.nprob) * G);
     CK(cudaMemcpy(res.data(), at<GroupResult>(p, P.o_results), res.size() * sizeof(GroupResult), cudaMemcpyDeviceToHost));

@@ -123,6 +123,21 @@ __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.comm
 __device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
+__device__ __forceinline__ float lds_f32(uint32_t a)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ double lds_f64(uint32_t a)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts_f32(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
+__device__ __forceinline__ void sts_f64(uint32_t a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
+
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p)
 {
     unsigned v;
@@ -154,8 +169,10 @@ __device__ __forceinline__ double rcp_f64(double d)
     return fma(r0, fma(e, e, e), r0);
 }
 
+// `act` = this lane holds a real cell; idle lanes of the warp-wavefront compute on stale values and
+// must not trigger fix-up passes.
 template <bool FIX>
-__device__ __forceinline__ float dd_cell(float q, double sig, double cx, double cy, double cz, double csum,
+__device__ __forceinline__ float dd_cell(bool act, float q, double sig, double cx, double cy, double cz, double csum,
                                          double a, double b, double c, double& ox, double& oy, double& oz)
 {
     const double ta = cx * a, tb = cy * b, tc = cz * c;
@@ -168,7 +185,7 @@ __device__ __forceinline__ float dd_cell(float q, double sig, double cx, double 
         bool fx = false, fy = false, fz = false;
 #pragma unroll 1
         for (int pass = 0; pass < 3; ++pass) {
-            const bool nx_ = !fx && ox < 0.0, ny_ = !fy && oy < 0.0, nz_ = !fz && oz < 0.0;
+            const bool nx_ = act && !fx && ox < 0.0, ny_ = act && !fy && oy < 0.0, nz_ = act && !fz && oz < 0.0;
             if (!(nx_ || ny_ || nz_)) break;
             fx |= nx_; fy |= ny_; fz |= nz_;
             double n2 = dq, d2 = sig;

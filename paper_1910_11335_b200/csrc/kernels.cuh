@@ -393,7 +393,7 @@ k_subsweep(MeshDev m, const int32_t* __restrict__ cells, int count, int octant, 
             double b = hy ? outy[fo + cuy] : 0.0;
             double cz = hz ? outz[fo + cuz] : 0.0;
             double ox, oy, oz;
-            float psi = dd_cell<FIX>(qn, sg, dcx, dcy, dcz, dcs, a, b, cz, ox, oy, oz);
+            float psi = dd_cell<FIX>(true, qn, sg, dcx, dcy, dcz, dcs, a, b, cz, ox, oy, oz);
             outx[fo + cp] = ox; outy[fo + cp] = oy; outz[fo + cp] = oz;
             const float4 lc = leakcoef[nd];
             if (bx) lk = fmaf(lc.x, (float)ox, lk);

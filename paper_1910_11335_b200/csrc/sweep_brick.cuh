@@ -48,6 +48,7 @@ struct BrickParams {
     const float4* leakcoef;      // [ndir] {w|mu|dy dz, w|eta|dx dz, w|xi|dx dy, 0}
     const ProbState* state;
     double* leak;                // [prob]
+    long long* dbg_time;         // -DDOCTORS_TIMING builds only: [16] cycle sums per phase (thread 0 of every CTA)
     int* dbg_plane;              // debug hook: NULL, or [BX*BY*BZ] receives the step at which each cell of a full brick is visited
 };
 
@@ -66,8 +67,8 @@ __host__ __device__ inline BrickSmem brick_smem_layout(int NM, int BX, int BY, i
     s.q = o;     o = align_up(o + size_t(NM > M ? NM : M) * NC * 4, 128);
     s.sig = o;   o = align_up(o + NC * 8, 128);
     s.psi = s.q;
-    s.fx = o;    o = align_up(o + size_t(M) * BY * BZ * 8, 16);
-    s.fy = o;    o = align_up(o + size_t(M) * BX * BZ * 8, 16);
+    s.fx = o;    o = align_up(o + size_t(M) * BY * BZ * 8, 8);      // fx, fy, fz contiguous (one load loop)
+    s.fy = o;    o = align_up(o + size_t(M) * BX * BZ * 8, 8);
     s.fz = o;    o = align_up(o + size_t(M) * BX * BY * 8, 16);
     s.dir = o;   o = align_up(o + size_t(M) * 32, 16);
     s.lk = o;    o = align_up(o + size_t(M) * 16, 16);
@@ -84,6 +85,7 @@ __device__ __forceinline__ void lane_cross_section(int lane, int BY, int& jp, in
     jp = lane % BY;
     kp = lane / BY;
 }
+constexpr int kFaceRegs = 7;
 __device__ __forceinline__ int step_to_ip(int s, int jp, int kp) { return s - jp - kp; }
 
 template <int NM, bool FIX, bool DBG = false>
@@ -121,12 +123,25 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
     const int faceXn = M * BY * BZ, faceYn = M * BX * BZ, faceZn = M * BX * BY;
     const int nbricks = P.gbx * P.gby * P.gbz;
     int last_oct = -1;
+#ifdef DOCTORS_TIMING
+    long long tacc[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0}, tprev = clock64();
+#define TICK(i) do { if (tid == 0) { long long t_ = clock64(); tacc[i] += t_ - tprev; tprev = t_; } } while (0)
+#else
+#define TICK(i) do { } while (0)
+#endif
 
+    // The id of the next task is fetched one task ahead (the atomic's round trip hides behind the
+    // sweep).  Holding one unstarted task cannot deadlock: a CTA's held task has a higher index than
+    // its running one, so the lowest unfinished task of the whole grid is always running.
+    if (tid == 0) sTask[0] = int(atomicAdd(&P.ctl->counters[P.counter_slot], 1u));
+    int slot = 0;
     while (true) {
-        if (tid == 0) *sTask = int(atomicAdd(&P.ctl->counters[P.counter_slot], 1u));
         __syncthreads();
-        const int t = *sTask;
+        const int t = sTask[slot];
         if (t >= P.ntasks) break;
+        if (tid == 32 % nthr) sTask[slot ^ 1] = int(atomicAdd(&P.ctl->counters[P.counter_slot], 1u));
+        slot ^= 1;
+        TICK(0);
         const uint2 td = P.tasks[P.task_begin + t];
         const int prob = td.x & 0xff, oct = (td.x >> 8) & 7;
         const int bi = td.y & 0x3ff, bj = (td.y >> 10) & 0x3ff, bk = (td.y >> 20) & 0x3ff;
@@ -153,10 +168,15 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
             mbar_expect_tx(bar, uint32_t(NM * NC * 4 + NC * 8));
             tma_load_5d(smem_u32(sQ), &tmQ, bar, x0, y0, z0, 0, prob);
             tma_load_3d(smem_u32(sSig), &tmSig, bar, x0, y0, z0);
-            // wait for the upwind bricks of this (problem, octant)
-            if (upx) while (ld_acquire_u32(flag_base + (brick - sx)) != P.epoch) __nanosleep(20);
-            if (upy) while (ld_acquire_u32(flag_base + (brick - sy * P.gbx)) != P.epoch) __nanosleep(20);
-            if (upz) while (ld_acquire_u32(flag_base + (brick - sz * P.gbx * P.gby)) != P.epoch) __nanosleep(20);
+        }
+        // wait for the upwind bricks of this (problem, octant): one warp-0 lane per upwind flag
+        if (warp == 0) {
+            const bool need = lane == 0 ? upx : (lane == 1 ? upy : (lane == 2 && upz));
+            const int up = lane == 0 ? brick - sx : (lane == 1 ? brick - sy * P.gbx : brick - sz * P.gbx * P.gby);
+            bool ready = !need;
+            while (!__all_sync(0xffffffffu, ready)) {
+                if (!ready) ready = ld_acquire_u32(flag_base + up) == P.epoch;
+            }
         }
         // octant tables (directions of this octant are contiguous: n = oct*M + m)
         if (oct != last_oct) {
@@ -169,14 +189,29 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
             last_oct = oct;
         }
         __syncthreads();                                         // flags seen by thread 0 -> everyone may read faces
+        TICK(1);
 
-        // inflow faces: upwind brick's outflow, or vacuum
-        for (int e = tid; e < faceXn; e += nthr) sFx[e] = upx ? __ldcg(gFx + e) : 0.0;
-        for (int e = tid; e < faceYn; e += nthr) sFy[e] = upy ? __ldcg(gFy + e) : 0.0;
-        for (int e = tid; e < faceZn; e += nthr) sFz[e] = upz ? __ldcg(gFz + e) : 0.0;
-
+        // inflow faces: upwind brick's outflow, or vacuum.  sFx, sFy, sFz are contiguous.
+        // The first kFaceRegs elements of every thread travel through registers: their global loads are
+        // issued here and land in shared memory only after phase 0, which hides the L2/HBM latency.
+        const int nxy = faceXn + faceYn, nall = nxy + faceZn;
+        double fv[kFaceRegs];
+#pragma unroll
+        for (int k = 0; k < kFaceRegs; ++k) {
+            const int e = tid + k * nthr;
+            const double* src = e < faceXn ? gFx + e : (e < nxy ? gFy + (e - faceXn) : gFz + (e - nxy));
+            const bool u = e < faceXn ? upx : (e < nxy ? upy : upz);
+            fv[k] = (e < nall && u) ? __ldcg(src) : 0.0;
+        }
+        for (int e = tid + kFaceRegs * nthr; e < nall; e += nthr) {
+            const double* src = e < faceXn ? gFx + e : (e < nxy ? gFy + (e - faceXn) : gFz + (e - nxy));
+            const bool u = e < faceXn ? upx : (e < nxy ? upy : upz);
+            sFx[e] = u ? __ldcg(src) : 0.0;
+        }
+        TICK(2);
         mbar_wait(bar, parity);
         parity ^= 1u;
+        TICK(3);
 
         // ---- phase 0: q_n = sum_lm Mtab[n][lm] Q_lm for every cell of the brick (a5) ----
         for (int c = tid; c < NC; c += nthr) {
@@ -191,7 +226,13 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
                 sPsi[n * NC + c] = a;                            // in place: this thread has read all of cell c
             }
         }
+#pragma unroll
+        for (int k = 0; k < kFaceRegs; ++k) {
+            const int e = tid + k * nthr;
+            if (e < nall) sFx[e] = fv[k];
+        }
         __syncthreads();
+        TICK(4);
 
         // ---- wavefront (a3 level 2, a4): warp = direction, lanes = (j',k'), step s -> plane i'+j'+k' = s ----
         const bool edge_x = !dnx, edge_y = !dny, edge_z = !dnz;  // outflow faces on the mesh boundary
@@ -201,43 +242,41 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         const int nsteps = ex + ey + ez - 2;
         const bool last_y = jp == ey - 1, last_z = kp == ez - 1;
         const int li0 = (sx > 0 ? 0 : ex - 1) - sx * (jp + kp);   // li at step 0 (i' = -(j'+k')), advanced by sx per step
+        const uint32_t row = uint32_t(BX * (lj + BY * lk_) + li0);
+        const bool first_y = jp == 0, first_z = kp == 0;
         for (int n = warp; n < M; n += P.W) {
             const double cx = sDir[4 * n], cy = sDir[4 * n + 1], cz = sDir[4 * n + 2], cs = sDir[4 * n + 3];
-            float* psi_row = sPsi + n * NC + BX * (lj + BY * lk_);
-            const double* sig_row = sSig + BX * (lj + BY * lk_);
             double* fxp = sFx + n * (BY * BZ) + lj + BY * lk_;
-            double* fyp = sFy + (n * BZ + lk_) * BX;
-            double* fzp = sFz + (n * BY + lj) * BX;
+            // running shared-memory addresses of this lane's cell: advanced by one cell (sx) per step
+            uint32_t pq = smem_u32(sPsi) + 4u * (uint32_t(n * NC) + row);
+            uint32_t ps = smem_u32(sSig) + 8u * row;
+            uint32_t py = smem_u32(sFy) + 8u * uint32_t((n * BZ + lk_) * BX + li0);
+            uint32_t pz = smem_u32(sFz) + 8u * uint32_t((n * BY + lj) * BX + li0);
+            const int d4 = 4 * sx, d8 = 8 * sx;
             double ax = lane_ok ? *fxp : 0.0, oy = 0.0, oz = 0.0;
-            int ip = -(jp + kp), li = li0;
+            int ip = lane_ok ? -(jp + kp) : -(1 << 29);          // clipped lanes never become active
 #pragma unroll 1
-            for (int s = 0; s < nsteps; ++s, ++ip, li += sx) {
-                const double uy = __shfl_up_sync(0xffffffffu, oy, 1);
-                const double uz = __shfl_up_sync(0xffffffffu, oz, BY);
-                const bool act = lane_ok && (unsigned)ip < (unsigned)ex;
+            for (int s = 0; s < nsteps; ++s) {
+                double b = __shfl_up_sync(0xffffffffu, oy, 1);
+                double cc = __shfl_up_sync(0xffffffffu, oz, BY);
+                const bool act = (unsigned)ip < (unsigned)ex;    // this lane's cell lies on sub-sweep plane s
                 float q = 0.0f;
-                double sg = 1.0, a = 0.0, b = 0.0, cc = 0.0;     // idle lanes compute on zeros (no fix-up passes)
-                if (act) {
-                    q = psi_row[li];
-                    sg = sig_row[li];
-                    a = ax;
-                    b = jp == 0 ? fyp[li] : uy;
-                    cc = kp == 0 ? fzp[li] : uz;
-                }
-                double ox, ty, tz;
-                const float psi = dd_cell<FIX>(q, sg, cx, cy, cz, cs, a, b, cc, ox, ty, tz);
-                oy = ty; oz = tz;
-                if (act) {
-                    psi_row[li] = psi;
-                    ax = ox;
-                    if (last_y) fyp[li] = ty;
-                    if (last_z) fzp[li] = tz;
-                    if (DBG) P.dbg_plane[li + BX * (lj + BY * lk_)] = s;
-                }
+                double sg = 1.0;
+                if (act) { q = lds_f32(pq); sg = lds_f64(ps); }
+                if (act && first_y) b = lds_f64(py);
+                if (act && first_z) cc = lds_f64(pz);
+                double ox;
+                const float psi = dd_cell<FIX>(act, q, sg, cx, cy, cz, cs, ax, b, cc, ox, oy, oz);
+                if (act) { sts_f32(pq, psi); ax = ox; }
+                if (act && last_y) sts_f64(py, oy);
+                if (act && last_z) sts_f64(pz, oz);
+                if (DBG && act) P.dbg_plane[(pq - smem_u32(sPsi)) / 4u - uint32_t(n * NC)] = s;
+                ++ip; pq += d4; ps += d8; py += d8; pz += d8;
             }
             if (lane_ok) *fxp = ax;
         }
         __syncthreads();
+        TICK(5);
 
         // leakage through the mesh boundary (balance report): sum of w |Omega_d| A_d psi_out over boundary faces
         if (edge_x | edge_y | edge_z) {
@@ -264,10 +303,10 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         if (dny) for (int e = tid; e < faceYn; e += nthr) __stcg(gFy + e, sFy[e]);
         if (dnz) for (int e = tid; e < faceZn; e += nthr) __stcg(gFz + e, sFz[e]);
         __syncthreads();
-        if (tid == 0) {
-            __threadfence();
-            st_release_u32(flag_base + brick, P.epoch);
+        if (tid == nthr - 1) {                                   // the thread with the least phase-2 work
+            st_release_u32(flag_base + brick, P.epoch);      // cumulative: covers the CTA's face stores (ordered by the barrier)
         }
+        TICK(6);
 
         // ---- phase 2: phi_lm += sum_n Dtab[n][lm] psi_n (Eq. 3, a5), tile -> sQ, TMA reduce-add ----
         for (int c = tid; c < NC; c += nthr) {
@@ -285,6 +324,7 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         }
         fence_proxy_async_smem();
         __syncthreads();
+        TICK(7);
         if (tid == 0) {
             tma_reduce_add_5d(&tmPhi, smem_u32(sQ), x0, y0, z0, 0, prob * P.Gs + P.g);
             bulk_commit();
@@ -296,6 +336,13 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         }
     }
     if (tid == 0) bulk_wait0();
+#ifdef DOCTORS_TIMING
+    if (tid == 0 && P.dbg_time) {
+        tacc[8] = clock64() - tprev;
+        for (int i = 0; i < 9; ++i) atomicAdd(reinterpret_cast<unsigned long long*>(P.dbg_time) + i, (unsigned long long)tacc[i]);
+    }
+#endif
+#undef TICK
 }
 
 }  // namespace doctors
