@@ -109,7 +109,7 @@ typedef struct {
     int deterministic;        /* 1: octants swept one after another, fixed summation order (bit-reproducible) */
     int source_chunk;         /* problems solved together (HBM capacity); 0 = all that fit the workspace */
     int sweep_mode;           /* 0 brick wavefront kernel (product path); 1 the paper's one-launch-per-sub-sweep scheme */
-    int brick[3];             /* sweep_mode 0: brick extents in cells; 0 = automatic.  brick[0] % 4 == 0 */
+    int brick[3];             /* sweep_mode 0: brick extents in cells; 0 = automatic.  brick[0] % 4 == 0, brick[1]*brick[2] <= 32 */
     int ctas_per_sm;          /* sweep_mode 0: persistent CTAs per SM; 0 = occupancy maximum */
     int check_window;         /* tolerance mode: iterations enqueued between host reads of the device flag; 0 = 12 */
 } doctors_solve_opts;
@@ -155,13 +155,19 @@ int doctors_get_uncollided_flux(doctors_problem* p, int source, int group, float
  * for the bit-exact check against the oracle.
  *   level 0: cells of the whole mesh in sub-sweep order (what sweep_mode 1 launches over)
  *   level 1: bricks of the brick grid in sub-sweep order (the task order of sweep_mode 0)
- *   level 2: cells of one full brick in sub-sweep order (the in-brick wavefront of sweep_mode 0),
- *            local index li + bx*(lj + by*lk)
+ *   level 2: cells of one full brick in sub-sweep order, local index li + bx*(lj + by*lk).  The kernel
+ *            needs no table at this level (lane (j',k') at step s updates i' = s - j' - k'); the planes it
+ *            actually visits are checked with doctors_debug_device_brick_steps
  * dims = extents the schedule runs over; plane_offset has dims[0]+dims[1]+dims[2]-1 entries,
  * cell_of has dims[0]*dims[1]*dims[2].  Uses opts->brick (NULL opts = automatic). */
 int doctors_debug_schedule_dims(doctors_problem* p, const doctors_solve_opts* opts, int level, int dims[3]);
 int doctors_debug_get_schedule(doctors_problem* p, const doctors_solve_opts* opts, int octant, int level,
                                int32_t* plane_offset, int32_t* cell_of);
+/* Device-side check of the in-brick wavefront (level 2): runs the product sweep kernel on one full
+ * bx x by x bz brick for `octant` and returns, per cell (local index li + bx*(lj + by*lk)), the step at
+ * which the kernel updated it.  By Eq. (8) that step must equal the cell's sub-sweep
+ * index i'+j'+k' in the octant's sweep-space coordinates.  Needs a CUDA device. */
+int doctors_debug_device_brick_steps(doctors_problem* p, int bx, int by, int bz, int octant, int32_t* step_of_cell);
 /* P(S) of Eq. (9) as the library evaluates it. */
 long long doctors_wavefront_size(int nx, int ny, int nz, int S);
 /* Projection tables the kernels use (fp32 copies of these doubles):

@@ -21,7 +21,7 @@ EXPORTS = [
     "doctors_set_mesh_materials", "doctors_set_xs", "doctors_set_quadrature", "doctors_set_quadrature_points",
     "doctors_get_quadrature", "doctors_set_source", "doctors_n_problems", "doctors_workspace_bytes",
     "doctors_set_workspace", "doctors_solve", "doctors_get_flux_moments", "doctors_get_uncollided_flux",
-    "doctors_debug_schedule_dims", "doctors_debug_get_schedule", "doctors_wavefront_size", "doctors_debug_get_tables",
+    "doctors_debug_schedule_dims", "doctors_debug_get_schedule", "doctors_debug_device_brick_steps", "doctors_wavefront_size", "doctors_debug_get_tables",
     "doctors_host_level_symmetric", "doctors_host_schedule", "doctors_host_projection_tables",
 ]
 
@@ -90,6 +90,7 @@ def load_library():
     L.doctors_debug_schedule_dims.argtypes = [vp, C.POINTER(CSolveOpts), C.c_int, ip]
     L.doctors_debug_get_schedule.argtypes = [vp, C.POINTER(CSolveOpts), C.c_int, C.c_int,
                                              C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
+    L.doctors_debug_device_brick_steps.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int32)]
     L.doctors_wavefront_size.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int]
     L.doctors_wavefront_size.restype = C.c_longlong
     L.doctors_debug_get_tables.argtypes = [vp, C.c_int, dp, dp]
@@ -322,6 +323,13 @@ class Problem:
         self._check(self._L.doctors_debug_get_schedule(self._h, C.byref(o), octant, level,
                                                        _ptr(off, C.c_int32), _ptr(cells, C.c_int32)))
         return d, off, cells
+
+    def debug_device_brick_steps(self, brick, octant):
+        """Step at which the sweep kernel updates each cell of one full brick: int32 [bz][by][bx]."""
+        bx, by, bz = brick
+        out = np.full(bx * by * bz, -1, dtype=np.int32)
+        self._check(self._L.doctors_debug_device_brick_steps(self._h, bx, by, bz, octant, _ptr(out, C.c_int32)))
+        return out.reshape(bz, by, bx)
 
     def debug_tables(self, pl_order):
         om, w = self.get_quadrature()

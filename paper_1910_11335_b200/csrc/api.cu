@@ -993,6 +993,66 @@ int copy_rows_out(doctors_problem* p, const float* src, float* out, int out_is_d
 }
 }  // namespace
 
+// Test hook: run the product sweep kernel (its debug instantiation) on ONE full brick of the given
+// shape and octant and report, per cell, the wavefront step at which the kernel updated it.
+extern "C" int doctors_debug_device_brick_steps(doctors_problem* p, int bx, int by, int bz, int octant, int32_t* step_of_cell)
+{
+    if (!p || !step_of_cell || octant < 0 || octant > 7) return DOCTORS_INVALID_ARG;
+    if (bx <= 0 || bx % 4 != 0 || bx > 64 || by <= 0 || bz <= 0 || by * bz > 32)
+        return fail(p, DOCTORS_INVALID_ARG, "brick: bx a multiple of 4 (<= 64), by * bz <= 32");
+    CK(cudaSetDevice(p->device));
+    const int NC = bx * by * bz;
+    const size_t smem = brick_smem_layout(1, bx, by, bz, 1).total;
+    // scratch: Q, phi (float), sigt (double), faces (double), tables, control
+    struct Scratch { float* Q; float* phi; double* sig; double* face; float* tab; double* dird; float4* lk; uint2* task;
+                     unsigned* flags; Control* ctl; ProbState* st; double* leak; int* planes; } S;
+    const size_t nface = size_t(by) * bz + size_t(bx) * bz + size_t(bx) * by;
+    char* base = nullptr;
+    const size_t bytes = 4096 + size_t(NC) * (4 + 4 + 8 + 4) + nface * 8 * 2 + 1024;
+    CK(cudaMalloc(&base, bytes));
+    CK(cudaMemset(base, 0, bytes));
+    size_t off = 0;
+    auto take = [&](size_t n) { char* r = base + off; off = align_up(off + n, 256); return r; };
+    S.Q = (float*)take(size_t(NC) * 4); S.phi = (float*)take(size_t(NC) * 4); S.sig = (double*)take(size_t(NC) * 8);
+    S.planes = (int*)take(size_t(NC) * 4); S.face = (double*)take(nface * 8);
+    S.tab = (float*)take(64); S.dird = (double*)take(8 * 32); S.lk = (float4*)take(8 * 16); S.task = (uint2*)take(16);
+    S.flags = (unsigned*)take(64); S.ctl = (Control*)take(sizeof(Control)); S.st = (ProbState*)take(sizeof(ProbState)); S.leak = (double*)take(8);
+    if (off > bytes) { cudaFree(base); return fail(p, DOCTORS_ALLOC, "debug scratch too small"); }
+    const uint2 task = make_uint2(uint32_t(octant) << 8, 0u);
+    double dd[32]; for (int i = 0; i < 32; ++i) dd[i] = (i % 4 == 3) ? 3.0 : 1.0;
+    float one[16]; for (int i = 0; i < 16; ++i) one[i] = 1.0f;
+    cudaMemcpy(S.task, &task, sizeof task, cudaMemcpyHostToDevice);
+    cudaMemcpy(S.dird, dd, sizeof dd, cudaMemcpyHostToDevice);
+    cudaMemcpy(S.tab, one, sizeof one, cudaMemcpyHostToDevice);
+    SweepLaunch SL;
+    cuuint64_t d5[5] = {cuuint64_t(bx), cuuint64_t(by), cuuint64_t(bz), 1, 1};
+    cuuint64_t s5[4] = {cuuint64_t(bx) * 4, cuuint64_t(bx) * by * 4, cuuint64_t(NC) * 4, cuuint64_t(NC) * 4};
+    cuuint64_t s3[2] = {cuuint64_t(bx) * 8, cuuint64_t(bx) * by * 8};
+    cuuint32_t b5[5] = {cuuint32_t(bx), cuuint32_t(by), cuuint32_t(bz), 1, 1};
+    int rc = make_tensor_map(p, &SL.tmQ, S.Q, 5, d5, s5, b5);
+    if (rc == DOCTORS_OK) rc = make_tensor_map(p, &SL.tmPhi, S.phi, 5, d5, s5, b5);
+    if (rc == DOCTORS_OK) rc = make_tensor_map(p, &SL.tmSig, S.sig, 3, d5, s3, b5, CU_TENSOR_MAP_DATA_TYPE_FLOAT64);
+    if (rc != DOCTORS_OK) { cudaFree(base); return rc; }
+    BrickParams& bp = SL.bp;
+    std::memset(&bp, 0, sizeof bp);
+    bp.nx = bx; bp.ny = by; bp.nz = bz; bp.BX = bx; bp.BY = by; bp.BZ = bz; bp.gbx = bp.gby = bp.gbz = 1;
+    bp.M = 1; bp.W = 1; bp.g = 0; bp.Gs = 1; bp.epoch = 1; bp.task_begin = 0; bp.ntasks = 1; bp.counter_slot = 0;
+    bp.tasks = S.task; bp.ctl = S.ctl; bp.flags = S.flags;
+    bp.faceX = S.face; bp.faceY = S.face + size_t(by) * bz; bp.faceZ = bp.faceY + size_t(bx) * bz;
+    bp.Mtab = S.tab; bp.Dtab = S.tab; bp.dird = S.dird + 4 * 0; bp.leakcoef = S.lk; bp.state = S.st; bp.leak = S.leak;
+    bp.dbg_time = nullptr; bp.dbg_plane = S.planes;
+    cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<1, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+    if (e == cudaSuccess) {
+        k_sweep_brick<1, false, true><<<1, 32, smem, p->stream>>>(SL.tmQ, SL.tmPhi, SL.tmSig, bp);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
+    if (e == cudaSuccess) e = cudaMemcpy(step_of_cell, S.planes, size_t(NC) * 4, cudaMemcpyDeviceToHost);
+    cudaFree(base);
+    if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "debug brick launch failed: %s", cudaGetErrorString(e));
+    return DOCTORS_OK;
+}
+
 extern "C" int doctors_get_flux_moments(doctors_problem* p, int problem, int group, int l_max, float* out, int out_is_device)
 {
     if (!p || !out) return DOCTORS_INVALID_ARG;

@@ -45,6 +45,25 @@ def test_schedule_bit_exact(pkg, orc, wl_fn, brick):
     p.close()
 
 
+@pytest.mark.parametrize("brick", [(16, 8, 4), (8, 4, 8), (4, 3, 5), (12, 32, 1), (4, 1, 1)])
+def test_device_wavefront_planes_bit_exact(pkg, orc, brick):
+    """Level 2 on the device: the step at which the sweep kernel itself updates each cell of a brick
+    equals the cell's sub-sweep index of Eq. (8) in the oracle's schedule, for all 8 octants, and every
+    plane holds exactly P(S) cells (Eq. 9)."""
+    p = pkg.problem_from_workload(make_config(0))
+    bx, by, bz = brick
+    for octant in range(8):
+        steps = p.debug_device_brick_steps(brick, octant).reshape(-1)
+        off, cells = orc.schedule(bx, by, bz, octant)
+        want = np.empty(bx * by * bz, dtype=np.int32)
+        for S in range(len(off) - 1):
+            want[cells[off[S]:off[S + 1]]] = S
+        assert np.array_equal(steps, want), (brick, octant)
+        assert np.array_equal(np.bincount(steps, minlength=len(off) - 1),
+                              [orc.wavefront_size(bx, by, bz, S) for S in range(len(off) - 1)])
+    p.close()
+
+
 def test_tables_match_oracle(pkg, orc):
     wl = make_config(1)
     p = pkg.problem_from_workload(wl)
@@ -71,7 +90,7 @@ def test_config0(pkg, orc, closure, mode, det):
 
 @pytest.mark.parametrize("closure", [0, 1])
 @pytest.mark.parametrize("kind", [1, 2])
-@pytest.mark.parametrize("brick", [None, (4, 3, 5), (8, 2, 2), (12, 10, 9)])
+@pytest.mark.parametrize("brick", [None, (4, 3, 5), (8, 2, 2), (12, 8, 4), (16, 4, 8), (4, 1, 32)])
 def test_ragged_p3(pkg, orc, closure, kind, brick):
     """12x10x9 mesh (px padding, clipped bricks in every axis), 4 materials, P3, S8, point / cone source."""
     wl = tiny_p3_case(kind=kind)
@@ -233,7 +252,7 @@ def test_config4_batched_properties(pkg):
     batch must equal the same problem solved alone."""
     wl = single_sweep_case(4, groups=(0, 20, 46), n_sources=4, fixed_iters=3)
     p, info = run_gpu(wl, closure=1, fixed_iters=3)
-    assert info["brick"] == (8, 8, 8) or info["brick"][0] % 4 == 0
+    assert info["brick"][0] % 4 == 0 and info["brick"][1] * info["brick"][2] <= 32
     for q in range(4):
         for g in range(3):
             src, col, leak = info["balance"][q, g]
