@@ -44,10 +44,14 @@ def measured_peak():
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def workload_for(idx):
-    from workloads import make_config
-    wl = make_config(idx)
-    return wl
+def workload_for(idx, slice_=False):
+    from workloads import make_config, single_sweep_case
+    if slice_:
+        # ncu slice (profiles/): full mesh and quadrature of the config, 2 sources, one mid-spectrum group,
+        # 2 sweeps -> 2 launches of the sweep kernel with a workspace small enough for ncu's replay
+        g = {0: 0, 1: 9, 2: 9, 3: 9, 4: 20}[idx]
+        return single_sweep_case(idx, groups=(g,), n_sources=2 if idx == 4 else 1, fixed_iters=2)
+    return make_config(idx)
 
 
 def algorithmic_bytes_per_cell_octant(nm, batch):
@@ -202,12 +206,12 @@ def run_gpu_arm(args):
     import paper_1910_11335_b200 as pkg
     pkg.load_library()                       # raises if the CUDA library is missing: no fallback
 
-    wl = workload_for(args.config)
+    wl = workload_for(args.config, args.slice)
     nm = (wl.L + 1) ** 2
     p = pkg.problem_from_workload(wl, device=dev)
     kw = dict(tol=wl.tol, max_iters=wl.max_iters, closure=args.closure,
               fixed_iters=(wl.fixed_iters if wl.fixed_iters else None))
-    if args.config == 4:
+    if args.config == 4 and not args.slice:
         kw["source_chunk"] = 4               # 2 chunks of 4: all-group moments of 8 sources exceed HBM
     flush = None
     if wl.cells * 33 * 4 * min(4, len(wl.sources)) <= 126e6:
@@ -274,6 +278,8 @@ def run_gpu_arm(args):
     # ---- roofline of the dominant kernel (k_sweep_brick) ----
     peak, peak_src = measured_peak()
     batch = min(4, len(wl.sources)) if wl.mode == 0 else 1
+    if args.slice:
+        args.no_cpu = True
     bytes_per = algorithmic_bytes_per_cell_octant(nm, batch)
     problem_sweeps = updates / (wl.cells * wl.n_dir)               # sum of K[s][g] over the timed steps
     alg_bytes = problem_sweeps * wl.cells * 8 * bytes_per
@@ -316,6 +322,7 @@ def main():
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs index (default 4, the largest)")
     ap.add_argument("--closure", type=int, default=1, help="0 pure diamond difference, 1 + set-to-zero fix-up (R2)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--slice", action="store_true", help="profiling slice of the config (see workload_for); not a bench number")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--traffic", type=float, default=None,
