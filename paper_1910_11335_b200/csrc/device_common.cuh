@@ -138,6 +138,15 @@ __device__ __forceinline__ double lds_f64(uint32_t a)
 __device__ __forceinline__ void sts_f32(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
 __device__ __forceinline__ void sts_f64(uint32_t a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
 
+__device__ __forceinline__ void sts_f32_if(bool p, uint32_t a, float v)
+{
+    asm volatile("{\n\t.reg .pred pp;\n\tsetp.ne.b32 pp, %0, 0;\n\t@pp st.shared.f32 [%1], %2;\n\t}" ::"r"((int)p), "r"(a), "f"(v) : "memory");
+}
+__device__ __forceinline__ void sts_f64_if(bool p, uint32_t a, double v)
+{
+    asm volatile("{\n\t.reg .pred pp;\n\tsetp.ne.b32 pp, %0, 0;\n\t@pp st.shared.f64 [%1], %2;\n\t}" ::"r"((int)p), "r"(a), "d"(v) : "memory");
+}
+
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p)
 {
     unsigned v;
@@ -171,6 +180,29 @@ __device__ __forceinline__ double rcp_f64(double d)
 
 // `act` = this lane holds a real cell; idle lanes of the warp-wavefront compute on stale values and
 // must not trigger fix-up passes.
+__device__ __forceinline__ double dd_fixup(double dq, double sig, double cx, double cy, double cz,
+                                        double ta, double tb, double tc, double a, double b, double c,
+                                        double& ox, double& oy, double& oz)
+{
+    bool fx = ox < 0.0, fy = oy < 0.0, fz = oz < 0.0;
+    double psi = 0.0;
+#pragma unroll 1
+    for (int pass = 0; pass < 3; ++pass) {
+        double n2 = dq, d2 = sig;
+        if (fx) n2 = fma(0.5, ta, n2); else { n2 += ta; d2 += cx; }
+        if (fy) n2 = fma(0.5, tb, n2); else { n2 += tb; d2 += cy; }
+        if (fz) n2 = fma(0.5, tc, n2); else { n2 += tc; d2 += cz; }
+        psi = n2 * rcp_f64(d2);
+        ox = fx ? 0.0 : fma(2.0, psi, -a);
+        oy = fy ? 0.0 : fma(2.0, psi, -b);
+        oz = fz ? 0.0 : fma(2.0, psi, -c);
+        const bool nx_ = !fx && ox < 0.0, ny_ = !fy && oy < 0.0, nz_ = !fz && oz < 0.0;
+        if (!(nx_ || ny_ || nz_)) break;
+        fx |= nx_; fy |= ny_; fz |= nz_;
+    }
+    return psi;
+}
+
 template <bool FIX>
 __device__ __forceinline__ float dd_cell(bool act, float q, double sig, double cx, double cy, double cz, double csum,
                                          double a, double b, double c, double& ox, double& oy, double& oz)
@@ -182,21 +214,9 @@ __device__ __forceinline__ float dd_cell(bool act, float q, double sig, double c
     oy = fma(2.0, psi, -b);
     oz = fma(2.0, psi, -c);
     if (FIX) {
-        bool fx = false, fy = false, fz = false;
-#pragma unroll 1
-        for (int pass = 0; pass < 3; ++pass) {
-            const bool nx_ = act && !fx && ox < 0.0, ny_ = act && !fy && oy < 0.0, nz_ = act && !fz && oz < 0.0;
-            if (!(nx_ || ny_ || nz_)) break;
-            fx |= nx_; fy |= ny_; fz |= nz_;
-            double n2 = dq, d2 = sig;
-            if (fx) n2 = fma(0.5, ta, n2); else { n2 += ta; d2 += cx; }
-            if (fy) n2 = fma(0.5, tb, n2); else { n2 += tb; d2 += cy; }
-            if (fz) n2 = fma(0.5, tc, n2); else { n2 += tc; d2 += cz; }
-            psi = n2 * rcp_f64(d2);
-            ox = fx ? 0.0 : fma(2.0, psi, -a);
-            oy = fy ? 0.0 : fma(2.0, psi, -b);
-            oz = fz ? 0.0 : fma(2.0, psi, -c);
-        }
+        // any negative outflow?  (sign bits; -0.0 takes the slow path too, which then changes nothing)
+        const int sgn = __double2hiint(ox) | __double2hiint(oy) | __double2hiint(oz);
+        if (act && sgn < 0) psi = dd_fixup(dq, sig, cx, cy, cz, ta, tb, tc, a, b, c, ox, oy, oz);
     }
     return (float)psi;
 }

@@ -62,6 +62,7 @@ __host__ __device__ inline BrickSmem brick_smem_layout(int NM, int BX, int BY, i
 {
     BrickSmem s;
     size_t NC = size_t(BX) * BY * BZ, o = 0;
+    s.misc = o;  o = align_up(o + 128, 128);   // mbarrier, task slots, reduction scratch; also the pad idle lanes may read
     // one tile of max(NM, M) planes holds, in turn, Q_lm (TMA load), psi_n (in place, per cell) and the
     // phi_lm contribution (in place again, TMA reduce-add source)
     s.q = o;     o = align_up(o + size_t(NM > M ? NM : M) * NC * 4, 128);
@@ -74,7 +75,7 @@ __host__ __device__ inline BrickSmem brick_smem_layout(int NM, int BX, int BY, i
     s.lk = o;    o = align_up(o + size_t(M) * 16, 16);
     s.mt = o;    o = align_up(o + size_t(M) * NM * 4, 16);
     s.dt = o;    o = align_up(o + size_t(M) * NM * 4, 16);
-    s.misc = o;  o = align_up(o + 128, 16);
+    o = align_up(o + 128, 16);                  // tail pad (idle lanes may read up to 10 cells past the tables' start)
     s.total = o;
     return s;
 }
@@ -244,33 +245,38 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         const int li0 = (sx > 0 ? 0 : ex - 1) - sx * (jp + kp);   // li at step 0 (i' = -(j'+k')), advanced by sx per step
         const uint32_t row = uint32_t(BX * (lj + BY * lk_) + li0);
         const bool first_y = jp == 0, first_z = kp == 0;
+        // Idle lanes (before / after their x range) load from wherever their running address points — always
+        // inside this CTA's shared memory, which starts with a 128-byte pad and ends with the tables — and
+        // compute on that garbage; only stores and the x-face register are predicated.  Clipped lanes
+        // (beyond ey / ez) stay parked on the tile's first cell.
+        const int d4 = lane_ok ? 4 * sx : 0, d8 = 2 * d4;
+        const int shy = BY;
         for (int n = warp; n < M; n += P.W) {
             const double cx = sDir[4 * n], cy = sDir[4 * n + 1], cz = sDir[4 * n + 2], cs = sDir[4 * n + 3];
             double* fxp = sFx + n * (BY * BZ) + lj + BY * lk_;
             // running shared-memory addresses of this lane's cell: advanced by one cell (sx) per step
-            uint32_t pq = smem_u32(sPsi) + 4u * (uint32_t(n * NC) + row);
-            uint32_t ps = smem_u32(sSig) + 8u * row;
-            uint32_t py = smem_u32(sFy) + 8u * uint32_t((n * BZ + lk_) * BX + li0);
-            uint32_t pz = smem_u32(sFz) + 8u * uint32_t((n * BY + lj) * BX + li0);
-            const int d4 = 4 * sx, d8 = 8 * sx;
+            uint32_t pq = smem_u32(sPsi) + (lane_ok ? 4u * (uint32_t(n * NC) + row) : 0u);
+            uint32_t ps = smem_u32(sSig) + (lane_ok ? 8u * row : 0u);
+            uint32_t py = smem_u32(sFy) + (lane_ok ? 8u * uint32_t((n * BZ + lk_) * BX + li0) : 0u);
+            uint32_t pz = smem_u32(sFz) + (lane_ok ? 8u * uint32_t((n * BY + lj) * BX + li0) : 0u);
             double ax = lane_ok ? *fxp : 0.0, oy = 0.0, oz = 0.0;
             int ip = lane_ok ? -(jp + kp) : -(1 << 29);          // clipped lanes never become active
 #pragma unroll 1
-            for (int s = 0; s < nsteps; ++s) {
+            for (int s = nsteps; s > 0; --s) {
                 double b = __shfl_up_sync(0xffffffffu, oy, 1);
-                double cc = __shfl_up_sync(0xffffffffu, oz, BY);
-                const bool act = (unsigned)ip < (unsigned)ex;    // this lane's cell lies on sub-sweep plane s
-                float q = 0.0f;
-                double sg = 1.0;
-                if (act) { q = lds_f32(pq); sg = lds_f64(ps); }
-                if (act && first_y) b = lds_f64(py);
-                if (act && first_z) cc = lds_f64(pz);
+                double cc = __shfl_up_sync(0xffffffffu, oz, shy);
+                const bool act = (unsigned)ip < (unsigned)ex;    // this lane's cell lies on the current sub-sweep plane
+                const float q = lds_f32(pq);
+                const double sg = lds_f64(ps);
+                if (first_y) b = lds_f64(py);
+                if (first_z) cc = lds_f64(pz);
                 double ox;
                 const float psi = dd_cell<FIX>(act, q, sg, cx, cy, cz, cs, ax, b, cc, ox, oy, oz);
-                if (act) { sts_f32(pq, psi); ax = ox; }
-                if (act && last_y) sts_f64(py, oy);
-                if (act && last_z) sts_f64(pz, oz);
-                if (DBG && act) P.dbg_plane[(pq - smem_u32(sPsi)) / 4u - uint32_t(n * NC)] = s;
+                sts_f32_if(act, pq, psi);
+                sts_f64_if(act && last_y, py, oy);
+                sts_f64_if(act && last_z, pz, oz);
+                if (act) ax = ox;
+                if (DBG && act) P.dbg_plane[(pq - smem_u32(sPsi)) / 4u - uint32_t(n * NC)] = nsteps - s;
                 ++ip; pq += d4; ps += d8; py += d8; pz += d8;
             }
             if (lane_ok) *fxp = ax;
