@@ -781,6 +781,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         bp.dird = at<double>(p, P.o_dird); bp.leakcoef = at<float4>(p, P.o_lk);
         bp.dbg_plane = nullptr;
         bp.dbg_time = nullptr;
+        bp.bulk_faces = (P.face_x_n % 2 == 0 && P.face_y_n % 2 == 0 && P.face_z_n % 2 == 0) ? 1 : 0;
 #ifdef DOCTORS_TIMING
         { static long long* dt = nullptr; if (!dt) { cudaMalloc(&dt, 16 * 8); } cudaMemset(dt, 0, 16 * 8); bp.dbg_time = dt; }
 #endif

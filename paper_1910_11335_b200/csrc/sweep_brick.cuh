@@ -48,6 +48,7 @@ struct BrickParams {
     const float4* leakcoef;      // [ndir] {w|mu|dy dz, w|eta|dx dz, w|xi|dx dy, 0}
     const ProbState* state;
     double* leak;                // [prob]
+    int bulk_faces;              // 1: all three face blocks are multiples of 16 bytes -> moved by bulk async copies (TMA unit)
     long long* dbg_time;         // -DDOCTORS_TIMING builds only: [16] cycle sums per phase (thread 0 of every CTA)
     int* dbg_plane;              // debug hook: NULL, or [BX*BY*BZ] receives the step at which each cell of a full brick is visited
 };
@@ -110,7 +111,7 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
     float* sD = reinterpret_cast<float*>(smem + L.dt);
     uint64_t* sBar = reinterpret_cast<uint64_t*>(smem + L.misc);
     int* sTask = reinterpret_cast<int*>(smem + L.misc + 8);
-    float* sRed = reinterpret_cast<float*>(smem + L.misc + 16);     // kMaxSweepWarps floats
+    float* sRed = reinterpret_cast<float*>(smem + L.misc + 64);     // kMaxSweepWarps floats
 
     const int tid = threadIdx.x, nthr = blockDim.x;
     const int lane = tid & 31, warp = tid >> 5;
@@ -118,7 +119,8 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
     int jp, kp;
     lane_cross_section(lane, BY, jp, kp);
 
-    if (tid == 0) { mbar_init(bar, 1); fence_mbar_init(); }
+    const uint32_t barF = bar + 32;                                  // faces (bulk copies) complete here
+    if (tid == 0) { mbar_init(bar, 1); mbar_init(barF, 1); fence_mbar_init(); }
     __syncthreads();
     uint32_t parity = 0;
     const int faceXn = M * BY * BZ, faceYn = M * BX * BZ, faceZn = M * BX * BY;
@@ -193,21 +195,36 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         TICK(1);
 
         // inflow faces: upwind brick's outflow, or vacuum.  sFx, sFy, sFz are contiguous.
-        // The first kFaceRegs elements of every thread travel through registers: their global loads are
-        // issued here and land in shared memory only after phase 0, which hides the L2/HBM latency.
         const int nxy = faceXn + faceYn, nall = nxy + faceZn;
         double fv[kFaceRegs];
+        if (P.bulk_faces) {
+            // one thread hands the three blocks to the TMA unit (1-D bulk copies, complete on barF);
+            // vacuum faces are zero-filled by the threads.  Nothing here waits: the data is needed after phase 0.
+            if (tid == 0) {
+                fence_proxy_async_all();                         // flags acquired (generic proxy) -> async-proxy reads
+                mbar_expect_tx(barF, uint32_t(8 * ((upx ? faceXn : 0) + (upy ? faceYn : 0) + (upz ? faceZn : 0))));
+                if (upx) bulk_load(smem_u32(sFx), gFx, uint32_t(8 * faceXn), barF);
+                if (upy) bulk_load(smem_u32(sFy), gFy, uint32_t(8 * faceYn), barF);
+                if (upz) bulk_load(smem_u32(sFz), gFz, uint32_t(8 * faceZn), barF);
+            }
+            if (!upx) for (int e = tid; e < faceXn; e += nthr) sFx[e] = 0.0;
+            if (!upy) for (int e = tid; e < faceYn; e += nthr) sFy[e] = 0.0;
+            if (!upz) for (int e = tid; e < faceZn; e += nthr) sFz[e] = 0.0;
+        } else {
+            // odd-sized blocks: the first kFaceRegs elements of every thread travel through registers (their
+            // loads are issued here and parked in shared memory after phase 0), the rest is copied directly
 #pragma unroll
-        for (int k = 0; k < kFaceRegs; ++k) {
-            const int e = tid + k * nthr;
-            const double* src = e < faceXn ? gFx + e : (e < nxy ? gFy + (e - faceXn) : gFz + (e - nxy));
-            const bool u = e < faceXn ? upx : (e < nxy ? upy : upz);
-            fv[k] = (e < nall && u) ? __ldcg(src) : 0.0;
-        }
-        for (int e = tid + kFaceRegs * nthr; e < nall; e += nthr) {
-            const double* src = e < faceXn ? gFx + e : (e < nxy ? gFy + (e - faceXn) : gFz + (e - nxy));
-            const bool u = e < faceXn ? upx : (e < nxy ? upy : upz);
-            sFx[e] = u ? __ldcg(src) : 0.0;
+            for (int k = 0; k < kFaceRegs; ++k) {
+                const int e = tid + k * nthr;
+                const double* src = e < faceXn ? gFx + e : (e < nxy ? gFy + (e - faceXn) : gFz + (e - nxy));
+                const bool u = e < faceXn ? upx : (e < nxy ? upy : upz);
+                fv[k] = (e < nall && u) ? __ldcg(src) : 0.0;
+            }
+            for (int e = tid + kFaceRegs * nthr; e < nall; e += nthr) {
+                const double* src = e < faceXn ? gFx + e : (e < nxy ? gFy + (e - faceXn) : gFz + (e - nxy));
+                const bool u = e < faceXn ? upx : (e < nxy ? upy : upz);
+                sFx[e] = u ? __ldcg(src) : 0.0;
+            }
         }
         TICK(2);
         mbar_wait(bar, parity);
@@ -227,10 +244,14 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
                 sPsi[n * NC + c] = a;                            // in place: this thread has read all of cell c
             }
         }
+        if (P.bulk_faces) {
+            mbar_wait(barF, parity ^ 1u);                         // same phase sequence as `bar` (flipped above)
+        } else {
 #pragma unroll
-        for (int k = 0; k < kFaceRegs; ++k) {
-            const int e = tid + k * nthr;
-            if (e < nall) sFx[e] = fv[k];
+            for (int k = 0; k < kFaceRegs; ++k) {
+                const int e = tid + k * nthr;
+                if (e < nall) sFx[e] = fv[k];
+            }
         }
         __syncthreads();
         TICK(4);
@@ -305,12 +326,21 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         }
 
         // ---- outflow faces to the downwind bricks, then publish the brick ----
-        if (dnx) for (int e = tid; e < faceXn; e += nthr) __stcg(gFx + e, sFx[e]);
-        if (dny) for (int e = tid; e < faceYn; e += nthr) __stcg(gFy + e, sFy[e]);
-        if (dnz) for (int e = tid; e < faceZn; e += nthr) __stcg(gFz + e, sFz[e]);
-        __syncthreads();
-        if (tid == nthr - 1) {                                   // the thread with the least phase-2 work
-            st_release_u32(flag_base + brick, P.epoch);      // cumulative: covers the CTA's face stores (ordered by the barrier)
+        if (P.bulk_faces) {
+            fence_proxy_async_smem();                            // lanes' face writes -> visible to the async proxy
+            __syncthreads();
+            if (tid == nthr - 1) {
+                if (dnx) bulk_store(gFx, smem_u32(sFx), uint32_t(8 * faceXn));
+                if (dny) bulk_store(gFy, smem_u32(sFy), uint32_t(8 * faceYn));
+                if (dnz) bulk_store(gFz, smem_u32(sFz), uint32_t(8 * faceZn));
+                bulk_commit();
+            }
+        } else {
+            if (dnx) for (int e = tid; e < faceXn; e += nthr) __stcg(gFx + e, sFx[e]);
+            if (dny) for (int e = tid; e < faceYn; e += nthr) __stcg(gFy + e, sFy[e]);
+            if (dnz) for (int e = tid; e < faceZn; e += nthr) __stcg(gFz + e, sFz[e]);
+            __syncthreads();
+            if (tid == nthr - 1) st_release_u32(flag_base + brick, P.epoch);   // cumulative: covers the CTA's face stores (ordered by the barrier)
         }
         TICK(6);
 
@@ -327,6 +357,11 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
             }
 #pragma unroll
             for (int lm = 0; lm < NM; ++lm) sQ[lm * NC + c] = pv[lm];
+        }
+        if (P.bulk_faces && tid == nthr - 1) {                   // this thread's phase-2 share is done: publish the brick
+            bulk_wait0();                                        // face blocks are in global memory
+            fence_proxy_async_all();
+            st_release_u32(flag_base + brick, P.epoch);
         }
         fence_proxy_async_smem();
         __syncthreads();
