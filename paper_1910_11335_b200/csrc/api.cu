@@ -33,7 +33,7 @@ struct GroupResult { int iters; int hit_max; float resid; float pad; double leak
 // Workspace layout for one choice of options.
 struct Plan {
     bool ok = false;
-    int px = 0; long long cells_p = 0;
+    long long cells_p = 0; int NCb = 0; int tm_inner = 0, tm_rows = 0;   // TMA box = tm_rows rows of tm_inner cells = one brick
     int nprob = 0, chunk = 0, nchunks = 0, nsrc = 0, nvol = 0;
     int G = 0, L = 0, NM = 0, ndir = 0, M = 0;
     int mode = 0, sweep_mode = 0, deterministic = 0;
@@ -44,7 +44,7 @@ struct Plan {
     // offsets
     size_t o_mat, o_rho, o_sigt_hat, o_sigs, o_spec, o_srcs, o_extvol, o_mtab, o_dtab, o_lk,
         o_sigt, o_Q, o_fixed, o_phi0old, o_phiall, o_phi0all, o_phiu, o_state, o_ctl, o_leak, o_bal,
-        o_results, o_fixediters, o_tasks, o_flags, o_fx, o_fy, o_fz, o_dird, o_dbg, o_sched, o_ox, o_oy, o_oz;
+        o_matd, o_rhod, o_scratch, o_results, o_fixediters, o_tasks, o_flags, o_fx, o_fy, o_fz, o_dird, o_dbg, o_sched, o_ox, o_oy, o_oz;
     size_t face_x_n = 0, face_y_n = 0, face_z_n = 0;
     size_t total = 0;
 };
@@ -74,6 +74,7 @@ struct doctors_problem {
     // result bookkeeping
     bool solved = false;
     Plan plan;
+    MeshDev mesh_dev;
     int last_chunk_first = 0, last_chunk_count = 0;
     CUresult (*encode)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                        const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -109,8 +110,8 @@ void auto_brick(int NM, int M, int nx, int ny, int nz, const int* req, int B[3])
     B[1] = std::min(8, ny);
     B[2] = std::min(32 / B[1], nz);
     if (B[2] < 4 && B[1] < ny) B[1] = std::min(32 / B[2], ny);
-    const int cand[4] = {16, 12, 8, 4};
-    for (int c = 0; c < 4; ++c) {
+    const int cand[5] = {20, 16, 12, 8, 4};        // 20 x 8 x 4 = 640 cells = 2 per thread of a 320-thread CTA, 3 CTAs per SM
+    for (int c = 0; c < 5; ++c) {
         B[0] = std::min(cand[c], (nx + 3) / 4 * 4);
         if (brick_smem_layout(NM, B[0], B[1], B[2], M).total <= 74 * 1024) break;
     }
@@ -120,8 +121,6 @@ void auto_brick(int NM, int M, int nx, int ny, int nz, const int* req, int B[3])
 Plan make_plan(const doctors_problem* p, const doctors_solve_opts* o, int chunk)
 {
     Plan P;
-    P.px = (p->nx + 3) / 4 * 4;
-    P.cells_p = (long long)P.px * p->ny * p->nz;
     P.nprob = nprob_of(p);
     P.nsrc = int(p->sources.size());
     P.chunk = std::max(1, std::min(chunk, P.nprob));
@@ -137,6 +136,12 @@ Plan make_plan(const doctors_problem* p, const doctors_solve_opts* o, int chunk)
     P.gb[1] = (p->ny + P.B[1] - 1) / P.B[1];
     P.gb[2] = (p->nz + P.B[2] - 1) / P.B[2];
     P.nbricks = (long long)P.gb[0] * P.gb[1] * P.gb[2];
+    P.NCb = P.B[0] * P.B[1] * P.B[2];
+    P.cells_p = P.nbricks * P.NCb;                              // brick-major storage, edge bricks padded
+    // one brick = NCb contiguous cells; a TMA box row holds at most 256 elements and must be a 16-byte multiple
+    P.tm_rows = 1;
+    while ((P.NCb / 4) % P.tm_rows != 0 || P.NCb / P.tm_rows > 256) ++P.tm_rows;
+    P.tm_inner = P.NCb / P.tm_rows;
     P.ntasks = P.nbricks * 8 * P.chunk;
     P.smem = brick_smem_layout(P.NM, P.B[0], P.B[1], P.B[2], P.M).total;
     { int dpw = (P.M + kMaxSweepWarps - 1) / kMaxSweepWarps; P.W = (P.M + dpw - 1) / dpw; }
@@ -149,6 +154,9 @@ Plan make_plan(const doctors_problem* p, const doctors_solve_opts* o, int chunk)
     (void)src_per_chunk;
     P.o_mat = take(cp);
     P.o_rho = take(cp * 4);
+    P.o_matd = take(size_t(p->nx) * p->ny * p->nz);              // dense copies for the ray tracer
+    P.o_rhod = take(size_t(p->nx) * p->ny * p->nz * 4);
+    P.o_scratch = take(size_t(p->nx) * p->ny * p->nz * 4 * nm);  // get_*: dense staging of one (problem, group)
     P.o_sigt_hat = take(size_t(p->n_mat_xs) * G * 8);
     P.o_sigs = take(size_t(p->n_mat_xs) * (P.L + 1) * G * G * 4);
     P.o_spec = take(size_t(P.nsrc) * G * 8);
@@ -639,24 +647,33 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
     p->plan = P;
     const int NM = P.NM, G = P.G, L = P.L, M = P.M;
     const size_t cp = size_t(P.cells_p);
-    const int nx = p->nx, ny = p->ny, nz = p->nz, px = P.px;
+    const int nx = p->nx, ny = p->ny, nz = p->nz;
 
     MeshDev md;
-    md.nx = nx; md.ny = ny; md.nz = nz; md.px = px; md.cells_p = P.cells_p;
+    md.nx = nx; md.ny = ny; md.nz = nz; md.cells_p = P.cells_p;
+    md.BX = P.B[0]; md.BY = P.B[1]; md.BZ = P.B[2]; md.gbx = P.gb[0]; md.gby = P.gb[1]; md.gbz = P.gb[2]; md.NCb = P.NCb;
+    p->mesh_dev = md;
     md.dx = p->dx; md.dy = p->dy; md.dz = p->dz;
     md.x0 = 0.5 * p->dx - 0.5 * nx * p->dx; md.y0 = 0.5 * p->dy - 0.5 * ny * p->dy; md.z0 = 0.5 * p->dz - 0.5 * nz * p->dz;
 
-    // ---- upload inputs and tables (pitched rows) ----
+    // ---- upload inputs and tables (brick-major order; padding cells: material 0, density 0) ----
+    // x-runs of one brick row are contiguous in both orders
+    auto to_bricks = [&](const auto* dense, auto* bricked) {
+        for (int k = 0; k < nz; ++k)
+            for (int j = 0; j < ny; ++j)
+                for (int i0 = 0; i0 < nx; i0 += P.B[0])
+                    std::memcpy(bricked + cell_index(md, i0, j, k), dense + (size_t)nx * (j + (size_t)ny * k) + i0,
+                                sizeof(*dense) * size_t(std::min(P.B[0], nx - i0)));
+    };
     {
         std::vector<uint8_t> hm(cp, 0);
         std::vector<float> hr(cp, 0.0f);
-        for (int k = 0; k < nz; ++k)
-            for (int j = 0; j < ny; ++j) {
-                std::memcpy(&hm[(size_t)px * (j + (size_t)ny * k)], &p->mat[(size_t)nx * (j + (size_t)ny * k)], nx);
-                std::memcpy(&hr[(size_t)px * (j + (size_t)ny * k)], &p->rho[(size_t)nx * (j + (size_t)ny * k)], size_t(nx) * 4);
-            }
+        to_bricks(p->mat.data(), hm.data());
+        to_bricks(p->rho.data(), hr.data());
         CK(cudaMemcpyAsync(at<uint8_t>(p, P.o_mat), hm.data(), cp, cudaMemcpyHostToDevice, st));
         CK(cudaMemcpyAsync(at<float>(p, P.o_rho), hr.data(), cp * 4, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(at<uint8_t>(p, P.o_matd), p->mat.data(), p->mat.size(), cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(at<float>(p, P.o_rhod), p->rho.data(), p->rho.size() * 4, cudaMemcpyHostToDevice, st));
         CK(cudaStreamSynchronize(st));
     }
     std::vector<float> sigs_f(p->sigs.begin(), p->sigs.end());
@@ -673,11 +690,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
             if (H.kind == 0) {
                 D.vol_slot = slot;
                 std::vector<float> hv(size_t(G) * cp, 0.0f);
-                for (int g = 0; g < G; ++g)
-                    for (int k = 0; k < nz; ++k)
-                        for (int j = 0; j < ny; ++j)
-                            std::memcpy(&hv[(size_t)g * cp + (size_t)px * (j + (size_t)ny * k)],
-                                        &H.volume[((size_t)g * nz + k) * ny * nx + (size_t)j * nx], size_t(nx) * 4);
+                for (int g = 0; g < G; ++g) to_bricks(H.volume.data() + (size_t)g * nx * ny * nz, hv.data() + (size_t)g * cp);
                 CK(cudaMemcpyAsync(at<float>(p, P.o_extvol) + (size_t)slot * G * cp, hv.data(), hv.size() * 4, cudaMemcpyHostToDevice, st));
                 CK(cudaStreamSynchronize(st));
                 ++slot;
@@ -748,16 +761,17 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
 
         // tensor maps over the pitched arrays (x fastest)
         {
-            cuuint64_t d5[5] = {cuuint64_t(nx), cuuint64_t(ny), cuuint64_t(nz), cuuint64_t(NM), cuuint64_t(P.chunk)};
-            cuuint64_t s5[4] = {cuuint64_t(px) * 4, cuuint64_t(px) * ny * 4, cuuint64_t(cp) * 4, cuuint64_t(cp) * NM * 4};
-            cuuint32_t b5[5] = {cuuint32_t(P.B[0]), cuuint32_t(P.B[1]), cuuint32_t(P.B[2]), cuuint32_t(NM), 1};
-            rc = make_tensor_map(p, &SL.tmQ, at<float>(p, P.o_Q), 5, d5, s5, b5);
+            // brick-major arrays: a brick's cells of one moment are tm_rows contiguous rows of tm_inner cells
+            cuuint64_t d4[4] = {cuuint64_t(P.tm_inner), cuuint64_t(P.tm_rows) * P.nbricks, cuuint64_t(NM), cuuint64_t(P.chunk)};
+            cuuint64_t s4[3] = {cuuint64_t(P.tm_inner) * 4, cuuint64_t(cp) * 4, cuuint64_t(cp) * NM * 4};
+            cuuint32_t b4[4] = {cuuint32_t(P.tm_inner), cuuint32_t(P.tm_rows), cuuint32_t(NM), 1};
+            rc = make_tensor_map(p, &SL.tmQ, at<float>(p, P.o_Q), 4, d4, s4, b4);
             if (rc != DOCTORS_OK) return rc;
-            d5[4] = cuuint64_t(P.chunk) * G;
-            rc = make_tensor_map(p, &SL.tmPhi, at<float>(p, P.o_phiall), 5, d5, s5, b5);
+            d4[3] = cuuint64_t(P.chunk) * G;
+            rc = make_tensor_map(p, &SL.tmPhi, at<float>(p, P.o_phiall), 4, d4, s4, b4);
             if (rc != DOCTORS_OK) return rc;
-            cuuint64_t s3[2] = {cuuint64_t(px) * 8, cuuint64_t(px) * ny * 8};
-            rc = make_tensor_map(p, &SL.tmSig, at<double>(p, P.o_sigt), 3, d5, s3, b5, CU_TENSOR_MAP_DATA_TYPE_FLOAT64);
+            cuuint64_t s2[1] = {cuuint64_t(P.tm_inner) * 8};
+            rc = make_tensor_map(p, &SL.tmSig, at<double>(p, P.o_sigt), 2, d4, s2, b4, CU_TENSOR_MAP_DATA_TYPE_FLOAT64);
             if (rc != DOCTORS_OK) return rc;
         }
         int max_ctas = 0;
@@ -772,7 +786,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         bp.nx = nx; bp.ny = ny; bp.nz = nz;
         bp.BX = P.B[0]; bp.BY = P.B[1]; bp.BZ = P.B[2];
         bp.gbx = P.gb[0]; bp.gby = P.gb[1]; bp.gbz = P.gb[2];
-        bp.M = M; bp.W = P.W; bp.g = 0; bp.Gs = G; bp.epoch = 0;
+        bp.M = M; bp.W = P.W; bp.g = 0; bp.Gs = G; bp.epoch = 0; bp.tm_rows = P.tm_rows;
         bp.tasks = at<uint2>(p, P.o_tasks);
         bp.ctl = at<Control>(p, P.o_ctl);
         bp.flags = at<unsigned>(p, P.o_flags);
@@ -823,7 +837,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         // a1: uncollided flux of the chunk's sources
         CK(cudaEventRecord(ev_a, st));
         k_raytrace<<<dim3(unsigned((P.cells_p + kRayThreads - 1) / kRayThreads), nsrc_c), kRayThreads, 0, st>>>(
-            md, at<uint8_t>(p, P.o_mat), at<float>(p, P.o_rho), at<SourceDev>(p, P.o_srcs), src0,
+            md, at<uint8_t>(p, P.o_matd), at<float>(p, P.o_rhod), at<SourceDev>(p, P.o_srcs), src0,
             at<double>(p, P.o_sigt_hat), at<double>(p, P.o_spec), p->n_mat_xs, G, phi_u_c);
         CK(cudaGetLastError());
         ++kernel_launches;
@@ -981,14 +995,17 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
 }
 
 namespace {
-// pitched device rows -> dense rows (host or device destination)
+// brick-major device fields -> dense [field][nz][ny][nx] rows (host or device destination)
 int copy_rows_out(doctors_problem* p, const float* src, float* out, int out_is_device, int n_fields)
 {
     const Plan& P = p->plan;
-    cudaError_t e = cudaMemcpy2DAsync(out, size_t(p->nx) * 4, src, size_t(P.px) * 4, size_t(p->nx) * 4,
-                                      size_t(p->ny) * p->nz * n_fields, out_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, p->stream);
-    if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "copy out failed: %s", cudaGetErrorString(e));
-    e = cudaStreamSynchronize(p->stream);
+    const size_t n = size_t(p->nx) * p->ny * p->nz * n_fields;
+    float* dst = out_is_device ? out : at<float>(p, P.o_scratch);
+    const int blocks = int(std::min<size_t>((n + 255) / 256, size_t(16) * p->num_sms));
+    k_unbrick<<<blocks, 256, 0, p->stream>>>(p->mesh_dev, src, dst, n_fields);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess && !out_is_device) e = cudaMemcpyAsync(out, dst, n * 4, cudaMemcpyDeviceToHost, p->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
     if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "copy out failed: %s", cudaGetErrorString(e));
     return DOCTORS_OK;
 }
@@ -1026,18 +1043,21 @@ extern "C" int doctors_debug_device_brick_steps(doctors_problem* p, int bx, int 
     cudaMemcpy(S.dird, dd, sizeof dd, cudaMemcpyHostToDevice);
     cudaMemcpy(S.tab, one, sizeof one, cudaMemcpyHostToDevice);
     SweepLaunch SL;
-    cuuint64_t d5[5] = {cuuint64_t(bx), cuuint64_t(by), cuuint64_t(bz), 1, 1};
-    cuuint64_t s5[4] = {cuuint64_t(bx) * 4, cuuint64_t(bx) * by * 4, cuuint64_t(NC) * 4, cuuint64_t(NC) * 4};
-    cuuint64_t s3[2] = {cuuint64_t(bx) * 8, cuuint64_t(bx) * by * 8};
-    cuuint32_t b5[5] = {cuuint32_t(bx), cuuint32_t(by), cuuint32_t(bz), 1, 1};
-    int rc = make_tensor_map(p, &SL.tmQ, S.Q, 5, d5, s5, b5);
-    if (rc == DOCTORS_OK) rc = make_tensor_map(p, &SL.tmPhi, S.phi, 5, d5, s5, b5);
-    if (rc == DOCTORS_OK) rc = make_tensor_map(p, &SL.tmSig, S.sig, 3, d5, s3, b5, CU_TENSOR_MAP_DATA_TYPE_FLOAT64);
+    int rows = 1;
+    while ((NC / 4) % rows != 0 || NC / rows > 256) ++rows;
+    const int inner = NC / rows;
+    cuuint64_t d4[4] = {cuuint64_t(inner), cuuint64_t(rows), 1, 1};
+    cuuint64_t s4[3] = {cuuint64_t(inner) * 4, cuuint64_t(NC) * 4, cuuint64_t(NC) * 4};
+    cuuint64_t s2[1] = {cuuint64_t(inner) * 8};
+    cuuint32_t b4[4] = {cuuint32_t(inner), cuuint32_t(rows), 1, 1};
+    int rc = make_tensor_map(p, &SL.tmQ, S.Q, 4, d4, s4, b4);
+    if (rc == DOCTORS_OK) rc = make_tensor_map(p, &SL.tmPhi, S.phi, 4, d4, s4, b4);
+    if (rc == DOCTORS_OK) rc = make_tensor_map(p, &SL.tmSig, S.sig, 2, d4, s2, b4, CU_TENSOR_MAP_DATA_TYPE_FLOAT64);
     if (rc != DOCTORS_OK) { cudaFree(base); return rc; }
     BrickParams& bp = SL.bp;
     std::memset(&bp, 0, sizeof bp);
     bp.nx = bx; bp.ny = by; bp.nz = bz; bp.BX = bx; bp.BY = by; bp.BZ = bz; bp.gbx = bp.gby = bp.gbz = 1;
-    bp.M = 1; bp.W = 1; bp.g = 0; bp.Gs = 1; bp.epoch = 1; bp.task_begin = 0; bp.ntasks = 1; bp.counter_slot = 0;
+    bp.M = 1; bp.W = 1; bp.tm_rows = rows; bp.g = 0; bp.Gs = 1; bp.epoch = 1; bp.task_begin = 0; bp.ntasks = 1; bp.counter_slot = 0;
     bp.tasks = S.task; bp.ctl = S.ctl; bp.flags = S.flags;
     bp.faceX = S.face; bp.faceY = S.face + size_t(by) * bz; bp.faceZ = bp.faceY + size_t(bx) * bz;
     bp.Mtab = S.tab; bp.Dtab = S.tab; bp.dird = S.dird + 4 * 0; bp.leakcoef = S.lk; bp.state = S.st; bp.leak = S.leak;
@@ -1071,7 +1091,6 @@ extern "C" int doctors_get_flux_moments(doctors_problem* p, int problem, int gro
         return fail(p, DOCTORS_NOT_RETAINED, "moments l > 0 of problem %d were overwritten by a later chunk", problem);
     const int q = problem - p->last_chunk_first;
     const int nmo = (l_max + 1) * (l_max + 1);
-    // rows of one moment are ny*nz rows of nx; successive moments are cells_p apart = px*ny*nz -> still uniform row pitch
     const float* src = at<float>(p, P.o_phiall) + ((size_t)q * P.G + group) * P.NM * cp;
     return copy_rows_out(p, src, out, out_is_device, nmo);
 }

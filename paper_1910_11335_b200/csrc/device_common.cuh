@@ -10,13 +10,36 @@ constexpr int kMaxMaterials = 16;
 constexpr int kMaxMoments = 16;       // P3
 constexpr int kMaxSweepWarps = 10;   // sweep CTA = one warp per direction of the octant (looped if M > 10)
 
+// Device storage order of every per-cell array is BRICK-MAJOR: cell (i,j,k) lives at
+//   cp = brick * NCb + li + BX*(lj + BY*lk),  brick = bi + gbx*(bj + gby*bk),  (bi,li) = divmod(i, BX) ...
+// so that the tile a sweep task loads (one brick, one moment) is ONE contiguous run of NCb*4 bytes
+// instead of BY*BZ rows of BX*4 bytes (64-byte rows made the TMA unit fetch whole 128-byte lines: 2x
+// read amplification on Q, measured in round 1).  Bricks at the mesh edge are padded with inert cells
+// (density 0, all fields 0).  The ray tracer alone also reads dense x-fastest copies of material / density.
 struct MeshDev {
     int nx, ny, nz;
-    int px;                 // row pitch in cells (nx rounded up to 4: 16-byte rows for TMA)
-    long long cells_p;      // px * ny * nz
+    int BX, BY, BZ;         // brick extents
+    int gbx, gby, gbz;      // brick grid
+    int NCb;                // cells per brick
+    long long cells_p;      // gbx*gby*gbz*NCb (padded cell count)
     double dx, dy, dz;
     double x0, y0, z0;      // centre of cell (0,0,0)
 };
+__host__ __device__ __forceinline__ long long cell_index(const MeshDev& m, int i, int j, int k)
+{
+    const int bi = i / m.BX, bj = j / m.BY, bk = k / m.BZ;
+    const int li = i - bi * m.BX, lj = j - bj * m.BY, lk = k - bk * m.BZ;
+    return (long long)(bi + m.gbx * (bj + m.gby * bk)) * m.NCb + li + m.BX * (lj + m.BY * lk);
+}
+// returns false for a padding cell
+__host__ __device__ __forceinline__ bool cell_ijk(const MeshDev& m, long long cp, int& i, int& j, int& k)
+{
+    const int brick = int(cp / m.NCb), local = int(cp - (long long)brick * m.NCb);
+    const int li = local % m.BX, t = local / m.BX, lj = t % m.BY, lk = t / m.BY;
+    const int bi = brick % m.gbx, u = brick / m.gbx, bj = u % m.gby, bk = u / m.gby;
+    i = bi * m.BX + li; j = bj * m.BY + lj; k = bk * m.BZ + lk;
+    return i < m.nx && j < m.ny && k < m.nz;
+}
 
 struct SourceDev {
     int kind;               // 0 volume, 1 point, 2 cone
@@ -87,6 +110,30 @@ __device__ __forceinline__ void tma_load_5d(uint32_t dst, const CUtensorMap* map
         " [%0], [%1, {%3, %4, %5, %6, %7}], [%2];"
         ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(bar),
           "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2, int c3)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes"
+        " [%0], [%1, {%3, %4, %5, %6}], [%2];"
+        ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes"
+        " [%0], [%1, {%3, %4}], [%2];"
+        ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(bar), "r"(c0), "r"(c1)
+        : "memory");
+}
+__device__ __forceinline__ void tma_reduce_add_4d(const CUtensorMap* map, uint32_t src, int c0, int c1, int c2, int c3)
+{
+    asm volatile(
+        "cp.reduce.async.bulk.tensor.4d.global.shared::cta.add.tile.bulk_group"
+        " [%0, {%2, %3, %4, %5}], [%1];"
+        ::"l"(reinterpret_cast<uint64_t>(map)), "r"(src), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
         : "memory");
 }
 __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, uint32_t bar,

@@ -16,7 +16,7 @@ namespace doctors {
 constexpr int kRayThreads = 128;
 
 __global__ void __launch_bounds__(kRayThreads)
-k_raytrace(MeshDev m, const uint8_t* __restrict__ mat, const float* __restrict__ rho,
+k_raytrace(MeshDev m, const uint8_t* __restrict__ mat /*dense [nz][ny][nx]*/, const float* __restrict__ rho /*dense*/,
            const SourceDev* __restrict__ srcs, int src0, const double* __restrict__ sigt_hat,
            const double* __restrict__ spectrum, int n_mat, int G, float* __restrict__ phi_u)
 {
@@ -25,12 +25,10 @@ k_raytrace(MeshDev m, const uint8_t* __restrict__ mat, const float* __restrict__
     const SourceDev src = srcs[src0 + s];
     long long cp = (long long)blockIdx.x * kRayThreads + threadIdx.x;
     if (cp >= m.cells_p) return;
-    int i = int(cp % m.px);
-    long long r = cp / m.px;
-    int j = int(r % m.ny), k = int(r / m.ny);
+    int i, j, k;
+    const bool real = cell_ijk(m, cp, i, j, k);
     float* out = phi_u + (size_t)s * G * m.cells_p + cp;
-    if (i >= m.nx) return;
-    if (src.kind == 0) {
+    if (!real || src.kind == 0) {
         for (int g = 0; g < G; ++g) out[(size_t)g * m.cells_p] = 0.0f;
         return;
     }
@@ -74,7 +72,7 @@ k_raytrace(MeshDev m, const uint8_t* __restrict__ mat, const float* __restrict__
             if (tmax[1] < tmax[a]) a = 1;
             if (tmax[2] < tmax[a]) a = 2;
             double tn = fmin(tmax[a], R);
-            size_t v = (size_t)idx[0] + (size_t)m.px * (idx[1] + (size_t)m.ny * idx[2]);
+            size_t v = (size_t)idx[0] + (size_t)m.nx * (idx[1] + (size_t)m.ny * idx[2]);
             if (tn > t) sA[mat[v]][tid] += (double)rho[v] * (tn - t);
             t = tn;
             // advance along the axis that was hit (no dynamic register indexing)
@@ -98,8 +96,7 @@ __global__ void k_sigt(MeshDev m, const uint8_t* __restrict__ mat, const float* 
 {
     long long cp = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (cp >= m.cells_p) return;
-    int i = int(cp % m.px);
-    sigt[cp] = i < m.nx ? (double)rho[cp] * sigt_hat[mat[cp] * G + g] : 0.0;
+    sigt[cp] = (double)rho[cp] * sigt_hat[mat[cp] * G + g];        // padding cells carry density 0
 }
 
 // Real harmonics of reading R4 in Cartesian form (fp32), l <= 3.
@@ -153,11 +150,10 @@ k_fixed_source(MeshDev m, const uint8_t* __restrict__ mat, const float* __restri
     const int p = blockIdx.y;
     long long cp = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (cp >= m.cells_p) return;
-    int i = int(cp % m.px);
-    long long r = cp / m.px;
-    int j = int(r % m.ny), k = int(r / m.ny);
+    int i, j, k;
+    const bool real = cell_ijk(m, cp, i, j, k);
     float* out = fixed + (size_t)p * NM * m.cells_p + cp;
-    if (i >= m.nx) {
+    if (!real) {
 #pragma unroll
         for (int lm = 0; lm < NM; ++lm) out[(size_t)lm * m.cells_p] = 0.0f;
         return;
@@ -228,16 +224,10 @@ k_update(MeshDev m, const uint8_t* __restrict__ mat, const float* __restrict__ r
     if (st[p].done) return;
     long long cp = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (cp >= m.cells_p) return;
-    const int i = int(cp % m.px);
     float* ph = phi + ((size_t)p * Gs + g) * NM * m.cells_p + cp;
     float* q = Q + (size_t)p * NM * m.cells_p + cp;
     const float* fx = fixed + (size_t)p * NM * m.cells_p + cp;
-    if (i >= m.nx) {
-#pragma unroll
-        for (int lm = 0; lm < NM; ++lm) { q[(size_t)lm * m.cells_p] = 0.0f; ph[(size_t)lm * m.cells_p] = 0.0f; }
-        return;
-    }
-    const float dens = rho[cp];
+    const float dens = rho[cp];                                   // padding cells: density 0, fixed 0 -> Q = 0
     const int mt = mat[cp];
     float sl[4];
 #pragma unroll
@@ -369,14 +359,14 @@ k_subsweep(MeshDev m, const int32_t* __restrict__ cells, int count, int octant, 
     if (t < count) {
         int c = cells[t];
         int i = c % m.nx, j = (c / m.nx) % m.ny, k = c / (m.nx * m.ny);
-        size_t cp = (size_t)i + (size_t)m.px * (j + (size_t)m.ny * k);
+        size_t cp = (size_t)cell_index(m, i, j, k);
         const int sx = (octant & 1) ? -1 : 1, sy = (octant & 2) ? -1 : 1, sz = (octant & 4) ? -1 : 1;
         const int iu = i - sx, ju = j - sy, ku = k - sz;
         const bool hx = iu >= 0 && iu < m.nx, hy = ju >= 0 && ju < m.ny, hz = ku >= 0 && ku < m.nz;
         const bool bx = i + sx < 0 || i + sx >= m.nx, by = j + sy < 0 || j + sy >= m.ny, bz = k + sz < 0 || k + sz >= m.nz;
-        const size_t cux = (size_t)iu + (size_t)m.px * (j + (size_t)m.ny * k);
-        const size_t cuy = (size_t)i + (size_t)m.px * (ju + (size_t)m.ny * k);
-        const size_t cuz = (size_t)i + (size_t)m.px * (j + (size_t)m.ny * ku);
+        const size_t cux = hx ? (size_t)cell_index(m, iu, j, k) : 0;
+        const size_t cuy = hy ? (size_t)cell_index(m, i, ju, k) : 0;
+        const size_t cuz = hz ? (size_t)cell_index(m, i, j, ku) : 0;
         const double sg = sigt[cp];
         float q[NM], acc[NM];
         const float* qp = Q + (size_t)p * NM * m.cells_p + cp;
@@ -409,6 +399,19 @@ k_subsweep(MeshDev m, const int32_t* __restrict__ cells, int count, int octant, 
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) lk += __shfl_xor_sync(0xffffffffu, lk, o);
     if ((threadIdx.x & 31) == 0 && lk != 0.0f) atomicAdd(leak + p, (double)lk);
+}
+
+// brick-major device order -> dense x-fastest [field][nz][ny][nx] (get_* calls)
+__global__ void __launch_bounds__(256)
+k_unbrick(MeshDev m, const float* __restrict__ src /*[fields][cells_p]*/, float* __restrict__ dst, int n_fields)
+{
+    const long long cells = (long long)m.nx * m.ny * m.nz;
+    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < cells * n_fields; c += (long long)gridDim.x * blockDim.x) {
+        const int f = int(c / cells);
+        const long long r = c - (long long)f * cells;
+        const int i = int(r % m.nx), j = int((r / m.nx) % m.ny), kk = int(r / ((long long)m.nx * m.ny));
+        dst[c] = src[(size_t)f * m.cells_p + cell_index(m, i, j, kk)];
+    }
 }
 
 }  // namespace doctors

@@ -31,6 +31,7 @@ struct BrickParams {
     int BX, BY, BZ;              // brick extents (BX % 4 == 0, BY * BZ <= 32)
     int gbx, gby, gbz;           // brick grid
     int M;                       // directions per octant
+    int tm_rows;                 // TMA box rows per brick (tensor-map coordinate 1 of brick b = tm_rows * b)
     int W;                       // sweep warps per CTA (blockDim.x = 32 W); warp w takes directions w, w+W, ...
     int g, Gs;                   // current group; group slots in the phi tensor map (coordinate 4 = prob*Gs + g)
     unsigned epoch;              // value that marks a brick done in this launch
@@ -169,8 +170,8 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         if (tid == 0) {
             bulk_wait_read0();                                   // previous tile's reduce has read sQ
             mbar_expect_tx(bar, uint32_t(NM * NC * 4 + NC * 8));
-            tma_load_5d(smem_u32(sQ), &tmQ, bar, x0, y0, z0, 0, prob);
-            tma_load_3d(smem_u32(sSig), &tmSig, bar, x0, y0, z0);
+            tma_load_4d(smem_u32(sQ), &tmQ, bar, 0, P.tm_rows * brick, 0, prob);
+            tma_load_2d(smem_u32(sSig), &tmSig, bar, 0, P.tm_rows * brick);
         }
         // wait for the upwind bricks of this (problem, octant): one warp-0 lane per upwind flag
         if (warp == 0) {
@@ -367,7 +368,7 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         __syncthreads();
         TICK(7);
         if (tid == 0) {
-            tma_reduce_add_5d(&tmPhi, smem_u32(sQ), x0, y0, z0, 0, prob * P.Gs + P.g);
+            tma_reduce_add_4d(&tmPhi, smem_u32(sQ), 0, P.tm_rows * brick, 0, prob * P.Gs + P.g);
             bulk_commit();
             if (edge_x | edge_y | edge_z) {
                 float s = 0.0f;
