@@ -75,8 +75,8 @@ __host__ __device__ inline BrickSmem brick_smem_layout(int NM, int BX, int BY, i
     s.fz = o;    o = align_up(o + size_t(M) * BX * BY * 8, 16);
     s.dir = o;   o = align_up(o + size_t(M) * 32, 16);
     s.lk = o;    o = align_up(o + size_t(M) * 16, 16);
-    s.mt = o;    o = align_up(o + size_t(M) * NM * 4, 16);
-    s.dt = o;    o = align_up(o + size_t(M) * NM * 4, 16);
+    s.mt = o;    o = align_up(o + size_t(M) * ((NM + 3) / 4 * 4) * 4, 16);
+    s.dt = o;    o = align_up(o + size_t(M) * ((NM + 3) / 4 * 4) * 4, 16);
     o = align_up(o + 128, 16);                  // tail pad (idle lanes may read up to 10 cells past the tables' start)
     s.total = o;
     return s;
@@ -89,6 +89,7 @@ __device__ __forceinline__ void lane_cross_section(int lane, int BY, int& jp, in
     kp = lane / BY;
 }
 constexpr int kFaceRegs = 7;
+template <int NM> __host__ __device__ constexpr int kTabPitch() { return (NM + 3) / 4 * 4; }   // table row pitch (16-byte rows)
 __device__ __forceinline__ int step_to_ip(int s, int jp, int kp) { return s - jp - kp; }
 
 template <int NM, bool FIX, bool DBG = false>
@@ -185,8 +186,9 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         // octant tables (directions of this octant are contiguous: n = oct*M + m)
         if (oct != last_oct) {
             for (int e = tid; e < M * NM; e += nthr) {
-                sM[e] = P.Mtab[(size_t)oct * M * NM + e];
-                sD[e] = P.Dtab[(size_t)oct * M * NM + e];
+                const int n = e / NM, lm = e - n * NM;
+                sM[n * kTabPitch<NM>() + lm] = P.Mtab[(size_t)oct * M * NM + e];
+                sD[n * kTabPitch<NM>() + lm] = P.Dtab[(size_t)oct * M * NM + e];
             }
             for (int e = tid; e < M * 4; e += nthr) sDir[e] = P.dird[(size_t)oct * M * 4 + e];
             for (int e = tid; e < M; e += nthr) sLk[e] = P.leakcoef[oct * M + e];
@@ -233,16 +235,37 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         TICK(3);
 
         // ---- phase 0: q_n = sum_lm Mtab[n][lm] Q_lm for every cell of the brick (a5) ----
-        for (int c = tid; c < NC; c += nthr) {
-            float qv[NM];
+        // Two cells per thread share every coefficient load (the phase is bound by the shared-memory pipe);
+        // packed fp32x2 FMAs (FFMA2, sm_100) accumulate even / odd moments in the halves of a register pair.
+        for (int c = tid; c < NC; c += 2 * nthr) {
+            const int c2 = c + nthr;
+            const bool two = c2 < NC;
+            if constexpr (NM >= 2) {
+                float2 qa[NM / 2], qb[NM / 2];
 #pragma unroll
-            for (int lm = 0; lm < NM; ++lm) qv[lm] = sQ[lm * NC + c];
-            for (int n = 0; n < M; ++n) {
-                const float* mt = sM + n * NM;
-                float a = 0.0f;
+                for (int k = 0; k < NM / 2; ++k) {
+                    qa[k] = make_float2(sQ[(2 * k) * NC + c], sQ[(2 * k + 1) * NC + c]);
+                    qb[k] = two ? make_float2(sQ[(2 * k) * NC + c2], sQ[(2 * k + 1) * NC + c2]) : make_float2(0.0f, 0.0f);
+                }
+                float qla = 0.0f, qlb = 0.0f;
+                if (NM & 1) { qla = sQ[(NM - 1) * NC + c]; qlb = two ? sQ[(NM - 1) * NC + c2] : 0.0f; }
+                for (int n = 0; n < M; ++n) {
+                    const float2* mt = reinterpret_cast<const float2*>(sM + n * kTabPitch<NM>());
+                    float2 a = make_float2(0.0f, 0.0f), b = make_float2(0.0f, 0.0f);
 #pragma unroll
-                for (int lm = 0; lm < NM; ++lm) a = fmaf(mt[lm], qv[lm], a);
-                sPsi[n * NC + c] = a;                            // in place: this thread has read all of cell c
+                    for (int k = 0; k < NM / 2; ++k) { const float2 m2 = mt[k]; a = __ffma2_rn(m2, qa[k], a); b = __ffma2_rn(m2, qb[k], b); }
+                    float ra = a.x + a.y, rb = b.x + b.y;
+                    if (NM & 1) { const float ml = sM[n * kTabPitch<NM>() + NM - 1]; ra = fmaf(ml, qla, ra); rb = fmaf(ml, qlb, rb); }
+                    sPsi[n * NC + c] = ra;                       // in place: this thread has read all of its cells
+                    if (two) sPsi[n * NC + c2] = rb;
+                }
+            } else {
+                const float qa0 = sQ[c], qb0 = two ? sQ[c2] : 0.0f;
+                for (int n = 0; n < M; ++n) {
+                    const float m0 = sM[n * kTabPitch<NM>()];
+                    sPsi[n * NC + c] = m0 * qa0;
+                    if (two) sPsi[n * NC + c2] = m0 * qb0;
+                }
             }
         }
         if (P.bulk_faces) {
@@ -346,18 +369,38 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         TICK(6);
 
         // ---- phase 2: phi_lm += sum_n Dtab[n][lm] psi_n (Eq. 3, a5), tile -> sQ, TMA reduce-add ----
-        for (int c = tid; c < NC; c += nthr) {
-            float pv[NM];
+        for (int c = tid; c < NC; c += 2 * nthr) {
+            const int c2 = c + nthr;
+            const bool two = c2 < NC;
+            if constexpr (NM >= 2) {
+                float2 pa[NM / 2], pb[NM / 2];
+                float pla = 0.0f, plb = 0.0f;
 #pragma unroll
-            for (int lm = 0; lm < NM; ++lm) pv[lm] = 0.0f;
-            for (int n = 0; n < M; ++n) {
-                const float* dt = sD + n * NM;
-                const float v = sPsi[n * NC + c];
+                for (int k = 0; k < NM / 2; ++k) { pa[k] = make_float2(0.0f, 0.0f); pb[k] = make_float2(0.0f, 0.0f); }
+                for (int n = 0; n < M; ++n) {
+                    const float2* dt = reinterpret_cast<const float2*>(sD + n * kTabPitch<NM>());
+                    const float va = sPsi[n * NC + c], vb = two ? sPsi[n * NC + c2] : 0.0f;
+                    const float2 va2 = make_float2(va, va), vb2 = make_float2(vb, vb);
 #pragma unroll
-                for (int lm = 0; lm < NM; ++lm) pv[lm] = fmaf(dt[lm], v, pv[lm]);
+                    for (int k = 0; k < NM / 2; ++k) { const float2 d2 = dt[k]; pa[k] = __ffma2_rn(d2, va2, pa[k]); pb[k] = __ffma2_rn(d2, vb2, pb[k]); }
+                    if (NM & 1) { const float dl = sD[n * kTabPitch<NM>() + NM - 1]; pla = fmaf(dl, va, pla); plb = fmaf(dl, vb, plb); }
+                }
+#pragma unroll
+                for (int k = 0; k < NM / 2; ++k) {
+                    sQ[(2 * k) * NC + c] = pa[k].x; sQ[(2 * k + 1) * NC + c] = pa[k].y;
+                    if (two) { sQ[(2 * k) * NC + c2] = pb[k].x; sQ[(2 * k + 1) * NC + c2] = pb[k].y; }
+                }
+                if (NM & 1) { sQ[(NM - 1) * NC + c] = pla; if (two) sQ[(NM - 1) * NC + c2] = plb; }
+            } else {
+                float pa0 = 0.0f, pb0 = 0.0f;
+                for (int n = 0; n < M; ++n) {
+                    const float d0 = sD[n * kTabPitch<NM>()];
+                    pa0 = fmaf(d0, sPsi[n * NC + c], pa0);
+                    if (two) pb0 = fmaf(d0, sPsi[n * NC + c2], pb0);
+                }
+                sQ[c] = pa0;
+                if (two) sQ[c2] = pb0;
             }
-#pragma unroll
-            for (int lm = 0; lm < NM; ++lm) sQ[lm * NC + c] = pv[lm];
         }
         if (P.bulk_faces && tid == nthr - 1) {                   // this thread's phase-2 share is done: publish the brick
             bulk_wait0();                                        // face blocks are in global memory
