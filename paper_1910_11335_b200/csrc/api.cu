@@ -950,9 +950,9 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
     if (P.sweep_mode == 0 && SL.bp.dbg_time) {
         long long h[16];
         cudaMemcpy(h, SL.bp.dbg_time, sizeof h, cudaMemcpyDeviceToHost);
-        const char* nm[9] = {"fetch", "dep-wait", "face-load", "tma-wait", "phase0", "wavefront", "face-store+release", "phase2", "tail"};
-        double tot = 0; for (int i = 0; i < 9; ++i) tot += double(h[i]);
-        for (int i = 0; i < 9; ++i) fprintf(stderr, "  [timing] %-20s %6.2f %%  %.3e cycles\n", nm[i], 100.0 * h[i] / tot, double(h[i]));
+        const char* nm[12] = {"fetch", "dep: tables+sync", "face-load", "tma-wait", "phase0", "wavefront", "face-store+release", "phase2", "tail", "dep: reduce-read wait + TMA issue", "dep: flag poll", "-"};
+        double tot = 0; for (int i = 0; i < 12; ++i) tot += double(h[i]);
+        for (int i = 0; i < 12; ++i) fprintf(stderr, "  [timing] %-20s %6.2f %%  %.3e cycles\n", nm[i], 100.0 * h[i] / tot, double(h[i]));
     }
 #endif
     // ---- results ----

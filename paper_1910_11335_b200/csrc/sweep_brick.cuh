@@ -129,7 +129,7 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
     const int nbricks = P.gbx * P.gby * P.gbz;
     int last_oct = -1;
 #ifdef DOCTORS_TIMING
-    long long tacc[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0}, tprev = clock64();
+    long long tacc[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, tprev = clock64();
 #define TICK(i) do { if (tid == 0) { long long t_ = clock64(); tacc[i] += t_ - tprev; tprev = t_; } } while (0)
 #else
 #define TICK(i) do { } while (0)
@@ -168,12 +168,28 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         double* gFy = P.faceY + (po * (P.gbx * P.gbz) + bi + P.gbx * bk) * (size_t)faceYn;
         double* gFz = P.faceZ + (po * (P.gbx * P.gby) + bi + P.gbx * bj) * (size_t)faceZn;
 
+        // octant tables (directions of this octant are contiguous: n = oct*M + m): loaded by warps 1.. while
+        // warp 0 issues the tile load and polls the flags, so that their global-load latency is hidden
+        if (oct != last_oct) {
+            const int tt = nthr > 32 ? tid - 32 : tid, tn = nthr > 32 ? nthr - 32 : nthr;
+            if (tt >= 0) {
+                for (int e = tt; e < M * NM; e += tn) {
+                    const int n = e / NM, lm = e - n * NM;
+                    sM[n * kTabPitch<NM>() + lm] = P.Mtab[(size_t)oct * M * NM + e];
+                    sD[n * kTabPitch<NM>() + lm] = P.Dtab[(size_t)oct * M * NM + e];
+                }
+                for (int e = tt; e < M * 4; e += tn) sDir[e] = P.dird[(size_t)oct * M * 4 + e];
+                for (int e = tt; e < M; e += tn) sLk[e] = P.leakcoef[oct * M + e];
+            }
+            last_oct = oct;
+        }
         if (tid == 0) {
             bulk_wait_read0();                                   // previous tile's reduce has read sQ
             mbar_expect_tx(bar, uint32_t(NM * NC * 4 + NC * 8));
             tma_load_4d(smem_u32(sQ), &tmQ, bar, 0, P.tm_rows * brick, 0, prob);
             tma_load_2d(smem_u32(sSig), &tmSig, bar, 0, P.tm_rows * brick);
         }
+        TICK(9);
         // wait for the upwind bricks of this (problem, octant): one warp-0 lane per upwind flag
         if (warp == 0) {
             const bool need = lane == 0 ? upx : (lane == 1 ? upy : (lane == 2 && upz));
@@ -183,17 +199,7 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
                 if (!ready) ready = ld_acquire_u32(flag_base + up) == P.epoch;
             }
         }
-        // octant tables (directions of this octant are contiguous: n = oct*M + m)
-        if (oct != last_oct) {
-            for (int e = tid; e < M * NM; e += nthr) {
-                const int n = e / NM, lm = e - n * NM;
-                sM[n * kTabPitch<NM>() + lm] = P.Mtab[(size_t)oct * M * NM + e];
-                sD[n * kTabPitch<NM>() + lm] = P.Dtab[(size_t)oct * M * NM + e];
-            }
-            for (int e = tid; e < M * 4; e += nthr) sDir[e] = P.dird[(size_t)oct * M * 4 + e];
-            for (int e = tid; e < M; e += nthr) sLk[e] = P.leakcoef[oct * M + e];
-            last_oct = oct;
-        }
+        TICK(10);
         __syncthreads();                                         // flags seen by thread 0 -> everyone may read faces
         TICK(1);
 
@@ -402,14 +408,14 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
                 if (two) sQ[c2] = pb0;
             }
         }
-        if (P.bulk_faces && tid == nthr - 1) {                   // this thread's phase-2 share is done: publish the brick
-            bulk_wait0();                                        // face blocks are in global memory
-            fence_proxy_async_all();
-            st_release_u32(flag_base + brick, P.epoch);
-        }
         fence_proxy_async_smem();
         __syncthreads();
         TICK(7);
+        if (P.bulk_faces && tid == nthr - 1) {                   // publish the brick; the others already start the next task
+            bulk_wait0();                                        // face blocks are in global memory (and read out of sFx..sFz)
+            fence_proxy_async_all();
+            st_release_u32(flag_base + brick, P.epoch);
+        }
         if (tid == 0) {
             tma_reduce_add_4d(&tmPhi, smem_u32(sQ), 0, P.tm_rows * brick, 0, prob * P.Gs + P.g);
             bulk_commit();
@@ -424,7 +430,7 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
 #ifdef DOCTORS_TIMING
     if (tid == 0 && P.dbg_time) {
         tacc[8] = clock64() - tprev;
-        for (int i = 0; i < 9; ++i) atomicAdd(reinterpret_cast<unsigned long long*>(P.dbg_time) + i, (unsigned long long)tacc[i]);
+        for (int i = 0; i < 12; ++i) atomicAdd(reinterpret_cast<unsigned long long*>(P.dbg_time) + i, (unsigned long long)tacc[i]);
     }
 #endif
 #undef TICK
