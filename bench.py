@@ -49,8 +49,13 @@ def workload_for(idx, slice_=False):
     if slice_:
         # ncu slice (profiles/): full mesh and quadrature of the config, 2 sources, one mid-spectrum group,
         # 2 sweeps -> 2 launches of the sweep kernel with a workspace small enough for ncu's replay
-        g = {0: 0, 1: 9, 2: 9, 3: 9, 4: 20}[idx]
+        g = {0: 0, 1: 9, 2: 9, 3: 9, 4: 20}.get(idx, 45)
         return single_sweep_case(idx, groups=(g,), n_sources=2 if idx == 4 else 1, fixed_iters=2)
+    if idx >= 5:
+        # the paper's own workload shapes (Table 2) on synthetic cross sections:
+        # 5 coarse single projection, 6 coarse CT (16 cone beams summed), 7 fine single, 8 fine CT
+        from workloads import paper_shaped
+        return paper_shaped(fine=idx >= 7, ct=idx in (6, 8))
     return make_config(idx)
 
 
@@ -118,6 +123,13 @@ def oracle_sample(idx):
     """Bounded sample of config idx the oracle finishes in ~10-30 s: full mesh and quadrature,
     first source, highest-energy group, ray trace + a fixed number of sweeps."""
     from workloads import single_sweep_case, make_config
+    if idx >= 5:
+        from workloads import paper_shaped
+        import copy
+        wl = paper_shaped(fine=idx >= 7, ct=idx in (6, 8), G=90 if idx < 7 else 2)
+        if idx >= 7:
+            wl.fixed_iters = 2
+        return wl, "%s: %s" % (wl.name, "all 90 groups to tolerance" if idx < 7 else "2 of 90 groups, 2 sweeps each")
     if idx <= 1:
         wl = make_config(idx)
         return wl, "%s: whole config (all groups, to tolerance)" % wl.name
@@ -319,7 +331,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=2)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs index (default 4, the largest)")
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs index 0..4 (default 4, the largest); 5..8 = the paper's own workload shapes (coarse/fine x single/CT)")
     ap.add_argument("--closure", type=int, default=1, help="0 pure diamond difference, 1 + set-to-zero fix-up (R2)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--slice", action="store_true", help="profiling slice of the config (see workload_for); not a bench number")

@@ -111,7 +111,8 @@ typedef struct {
     int sweep_mode;           /* 0 brick wavefront kernel (product path); 1 the paper's one-launch-per-sub-sweep scheme */
     int brick[3];             /* sweep_mode 0: brick extents in cells; 0 = automatic.  brick[0] % 4 == 0, brick[1]*brick[2] <= 32 */
     int ctas_per_sm;          /* sweep_mode 0: persistent CTAs per SM; 0 = occupancy maximum */
-    int check_window;         /* tolerance mode: iterations enqueued between host reads of the device flag; 0 = 12 */
+    int check_window;         /* tolerance mode: sweeps enqueued between host reads of the device flag; 0 = adaptive
+                               * (first read one sweep before the count the previous group needed, then every sweep) */
 } doctors_solve_opts;
 
 typedef struct {

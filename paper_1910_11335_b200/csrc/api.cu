@@ -628,6 +628,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
     if (opts_in) o = *opts_in;
     if (!(o.tol > 0.0)) o.tol = 1e-5;
     if (o.max_iters <= 0) o.max_iters = 100;
+    const bool adaptive_window = o.check_window <= 0;   // first host read where the previous group stopped, then every sweep
     if (o.check_window <= 0) o.check_window = 12;
     if (o.closure != 0 && o.closure != 1) return fail(p, DOCTORS_INVALID_ARG, "closure must be 0 or 1");
     if (o.sweep_mode != 0 && o.sweep_mode != 1) return fail(p, DOCTORS_INVALID_ARG, "sweep_mode must be 0 or 1");
@@ -845,6 +846,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         CK(cudaEventSynchronize(ev_b));
         { float ms = 0; cudaEventElapsedTime(&ms, ev_a, ev_b); ms_ray += ms; }
 
+        int prev_group_iters = 0;                                 // sweeps the previous group of this chunk needed
         for (int g = 0; g < G; ++g) {
             k_group_begin<<<1, 256, 0, st>>>(at<ProbState>(p, P.o_state), at<Control>(p, P.o_ctl), at<int>(p, P.o_fixediters),
                                               prob0, nq, P.chunk, G, g, at<double>(p, P.o_bal));
@@ -876,7 +878,9 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
             CK(cudaEventRecord(i0, st));
             int k = 0;
             while (k < limit) {
-                const int batch = all_fixed ? limit : std::min(o.check_window, limit - k);
+                int batch = all_fixed ? limit : std::min(o.check_window, limit - k);
+                if (!all_fixed && adaptive_window)
+                    batch = std::min(limit - k, k == 0 ? (prev_group_iters > 1 ? prev_group_iters - 1 : std::min(o.check_window, 6)) : 1);
                 for (int b = 0; b < batch; ++b, ++k) {
 #define LAUNCH_UPDATE(NMv)                                                                                          \
     k_update<NMv><<<dim3(cblocks, nq), 256, 0, st>>>(md, at<uint8_t>(p, P.o_mat), at<float>(p, P.o_rho), at<float>(p, P.o_sigs), \
@@ -930,6 +934,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
                 CK(cudaStreamSynchronize(st));
                 if (*h_flag) break;
             }
+            prev_group_iters = k;
             CK(cudaEventRecord(i1, st));
             k_balance<<<dim3(red_blocks, nq), 256, 0, st>>>(md, g, G, NM, at<float>(p, P.o_phiall), at<float>(p, P.o_Q), at<double>(p, P.o_sigt),
                                                              p->dx * p->dy * p->dz, at<double>(p, P.o_bal));

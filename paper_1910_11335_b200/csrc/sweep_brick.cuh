@@ -97,6 +97,7 @@ __global__ void __launch_bounds__(32 * kMaxSweepWarps, 3)
 k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmPhi,
               const __grid_constant__ CUtensorMap tmSig, const BrickParams P)
 {
+    if (__ldcg(&P.ctl->all_done)) return;                              // every problem of the chunk has stopped (a6): nothing to sweep
     extern __shared__ __align__(128) unsigned char smem[];
     const int BX = P.BX, BY = P.BY, BZ = P.BZ, M = P.M;
     const int NC = BX * BY * BZ;
