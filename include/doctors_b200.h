@@ -113,6 +113,9 @@ typedef struct {
     int ctas_per_sm;          /* sweep_mode 0: persistent CTAs per SM; 0 = occupancy maximum */
     int check_window;         /* tolerance mode: sweeps enqueued between host reads of the device flag; 0 = adaptive
                                * (first read one sweep before the count the previous group needed, then every sweep) */
+    int projection;           /* sweep_mode 0, the two projections of Eq. (2) rhs / Eq. (3) inside the sweep kernel:
+                               * 0 automatic = tensor cores (mma TF32, 3-product split, fp32 accumulate) when P3 and the
+                               * octant has <= 48 directions, else packed fp32 FMA loops; 1 = always the fp32 FMA loops */
 } doctors_solve_opts;
 
 typedef struct {
@@ -126,6 +129,7 @@ typedef struct {
     int n_chunks;
     int brick[3];
     int ctas_per_sm;
+    int projection_mtiles;    /* > 0: the projections ran on the tensor cores (16-direction m-tiles per octant); 0: fp32 FMA loops */
 } doctors_solve_info;
 
 /* n_problems = n_sources (mode 0) or 1 (mode 1). */

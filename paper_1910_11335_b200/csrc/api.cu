@@ -33,7 +33,8 @@ struct GroupResult { int iters; int hit_max; float resid; float pad; double leak
 // Workspace layout for one choice of options.
 struct Plan {
     bool ok = false;
-    long long cells_p = 0; int NCb = 0; int tm_inner = 0, tm_rows = 0;   // TMA box = tm_rows rows of tm_inner cells = one brick
+    long long cells_p = 0; int NCb = 0;
+    int MT = 0;                     // m-tiles of the tensor-core projections (0: FFMA2 loops), see sweep_brick.cuh
     int nprob = 0, chunk = 0, nchunks = 0, nsrc = 0, nvol = 0;
     int G = 0, L = 0, NM = 0, ndir = 0, M = 0;
     int mode = 0, sweep_mode = 0, deterministic = 0;
@@ -44,7 +45,7 @@ struct Plan {
     // offsets
     size_t o_mat, o_rho, o_sigt_hat, o_sigs, o_spec, o_srcs, o_extvol, o_mtab, o_dtab, o_lk,
         o_sigt, o_Q, o_fixed, o_phi0old, o_phiall, o_phi0all, o_phiu, o_state, o_ctl, o_leak, o_bal,
-        o_matd, o_rhod, o_scratch, o_results, o_fixediters, o_tasks, o_flags, o_fx, o_fy, o_fz, o_dird, o_dbg, o_sched, o_ox, o_oy, o_oz;
+        o_matd, o_rhod, o_scratch, o_results, o_fixediters, o_tasks, o_flags, o_fx, o_fy, o_fz, o_dird, o_dbg, o_sched, o_ox, o_oy, o_oz, o_octtab;
     size_t face_x_n = 0, face_y_n = 0, face_z_n = 0;
     size_t total = 0;
 };
@@ -113,7 +114,7 @@ void auto_brick(int NM, int M, int nx, int ny, int nz, const int* req, int B[3])
     const int cand[5] = {20, 16, 12, 8, 4};        // 20 x 8 x 4 = 640 cells = 2 per thread of a 320-thread CTA, 3 CTAs per SM
     for (int c = 0; c < 5; ++c) {
         B[0] = std::min(cand[c], (nx + 3) / 4 * 4);
-        if (brick_smem_layout(NM, B[0], B[1], B[2], M).total <= 74 * 1024) break;
+        if (brick_smem_layout(NM, B[0], B[1], B[2], M, projection_mtiles(NM, M, B[0] * B[1] * B[2])).total <= 74 * 1024) break;
     }
 }
 
@@ -138,12 +139,10 @@ Plan make_plan(const doctors_problem* p, const doctors_solve_opts* o, int chunk)
     P.nbricks = (long long)P.gb[0] * P.gb[1] * P.gb[2];
     P.NCb = P.B[0] * P.B[1] * P.B[2];
     P.cells_p = P.nbricks * P.NCb;                              // brick-major storage, edge bricks padded
-    // one brick = NCb contiguous cells; a TMA box row holds at most 256 elements and must be a 16-byte multiple
-    P.tm_rows = 1;
-    while ((P.NCb / 4) % P.tm_rows != 0 || P.NCb / P.tm_rows > 256) ++P.tm_rows;
-    P.tm_inner = P.NCb / P.tm_rows;
+    // one brick = NCb contiguous cells per moment: moved by 1-D bulk copies (16-byte multiples: BX % 4 == 0)
     P.ntasks = P.nbricks * 8 * P.chunk;
-    P.smem = brick_smem_layout(P.NM, P.B[0], P.B[1], P.B[2], P.M).total;
+    P.MT = (o && o->projection == 1) ? 0 : projection_mtiles(P.NM, P.M, P.NCb);
+    P.smem = brick_smem_layout(P.NM, P.B[0], P.B[1], P.B[2], P.M, P.MT).total;
     { int dpw = (P.M + kMaxSweepWarps - 1) / kMaxSweepWarps; P.W = (P.M + dpw - 1) / dpw; }
 
     size_t off = 0;
@@ -189,13 +188,14 @@ Plan make_plan(const doctors_problem* p, const doctors_solve_opts* o, int chunk)
         P.o_fy = take(size_t(P.chunk) * 8 * P.gb[0] * P.gb[2] * P.face_y_n * 8);
         P.o_fz = take(size_t(P.chunk) * 8 * P.gb[0] * P.gb[1] * P.face_z_n * 8);
         P.o_dbg = take(size_t(P.B[0]) * P.B[1] * P.B[2] * 4);
+        P.o_octtab = take(8 * octtab_layout(P.NM, P.M, P.MT).total);
         P.o_sched = P.o_ox = P.o_oy = P.o_oz = 0;
     } else {
         P.o_sched = take(size_t(8) * p->nx * p->ny * p->nz * 4);
         P.o_ox = take(size_t(P.chunk) * P.M * cp * 8);
         P.o_oy = take(size_t(P.chunk) * P.M * cp * 8);
         P.o_oz = take(size_t(P.chunk) * P.M * cp * 8);
-        P.o_tasks = P.o_flags = P.o_fx = P.o_fy = P.o_fz = P.o_dbg = 0;
+        P.o_tasks = P.o_flags = P.o_fx = P.o_fy = P.o_fz = P.o_dbg = P.o_octtab = 0;
     }
     P.total = off;
     P.ok = true;
@@ -576,45 +576,104 @@ int make_tensor_map(doctors_problem* p, CUtensorMap* tm, void* base, int rank, c
 }
 
 struct SweepLaunch {
-    CUtensorMap tmQ, tmPhi, tmSig;
     BrickParams bp;
     int grid = 0;
     size_t smem = 0;
 };
 
-template <int NM, bool FIX>
+template <int NM, bool FIX, int MT>
 cudaError_t launch_brick(const SweepLaunch& S, cudaStream_t st)
 {
-    k_sweep_brick<NM, FIX><<<S.grid, 32 * S.bp.W, S.smem, st>>>(S.tmQ, S.tmPhi, S.tmSig, S.bp);
+    k_sweep_brick<NM, FIX, MT><<<S.grid, 32 * S.bp.W, S.smem, st>>>(S.bp);
     return cudaGetLastError();
 }
 
-template <int NM, bool FIX>
+template <int NM, bool FIX, int MT>
 cudaError_t prep_brick(size_t smem, int threads, int* max_ctas)
 {
-    cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<NM, FIX>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+    cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<NM, FIX, MT>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(max_ctas, k_sweep_brick<NM, FIX>, threads, smem);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(max_ctas, k_sweep_brick<NM, FIX, MT>, threads, smem);
 }
 
-#define DISPATCH_NM_FIX(NMv, FIXv, EXPR)                                         \
+// NM in {1, 4, 9, 16}; MT > 0 only with NM = 16 (projection_mtiles)
+#define DISPATCH_ONE(NMc, FIXc, MTc, EXPR) { constexpr int NM = NMc; constexpr bool FIX = FIXc; constexpr int MT = MTc; EXPR; }
+#define DISPATCH_NM(NMv, FIXc, MTv, EXPR)                                        \
+    switch (NMv) {                                                               \
+        case 1: DISPATCH_ONE(1, FIXc, 0, EXPR) break;                            \
+        case 4: DISPATCH_ONE(4, FIXc, 0, EXPR) break;                            \
+        case 9: DISPATCH_ONE(9, FIXc, 0, EXPR) break;                            \
+        default:                                                                 \
+            switch (MTv) {                                                       \
+                case 1: DISPATCH_ONE(16, FIXc, 1, EXPR) break;                   \
+                case 2: DISPATCH_ONE(16, FIXc, 2, EXPR) break;                   \
+                case 3: DISPATCH_ONE(16, FIXc, 3, EXPR) break;                   \
+                default: DISPATCH_ONE(16, FIXc, 0, EXPR) break;                  \
+            }                                                                    \
+            break;                                                               \
+    }
+#define DISPATCH_NM_FIX(NMv, FIXv, MTv, EXPR)                                    \
     do {                                                                         \
-        if (FIXv) {                                                              \
-            switch (NMv) {                                                       \
-                case 1: { constexpr int NM = 1; constexpr bool FIX = true; EXPR; } break;   \
-                case 4: { constexpr int NM = 4; constexpr bool FIX = true; EXPR; } break;   \
-                case 9: { constexpr int NM = 9; constexpr bool FIX = true; EXPR; } break;   \
-                default: { constexpr int NM = 16; constexpr bool FIX = true; EXPR; } break; \
-            }                                                                    \
-        } else {                                                                 \
-            switch (NMv) {                                                       \
-                case 1: { constexpr int NM = 1; constexpr bool FIX = false; EXPR; } break;  \
-                case 4: { constexpr int NM = 4; constexpr bool FIX = false; EXPR; } break;  \
-                case 9: { constexpr int NM = 9; constexpr bool FIX = false; EXPR; } break;  \
-                default: { constexpr int NM = 16; constexpr bool FIX = false; EXPR; } break;\
-            }                                                                    \
-        }                                                                        \
+        if (FIXv) { DISPATCH_NM(NMv, true, MTv, EXPR) } else { DISPATCH_NM(NMv, false, MTv, EXPR) } \
     } while (0)
+
+// TF32 rounding (round to nearest, ties away: what cvt.rna.tf32.f32 does) for the pre-split coefficient fragments
+inline float tf32_rna(float v)
+{
+    uint32_t u; std::memcpy(&u, &v, 4);
+    u = (u + 0x1000u) & 0xffffe000u;
+    float r; std::memcpy(&r, &u, 4);
+    return r;
+}
+
+// The per-octant table blobs of octtab_layout(): direction coefficients, leakage coefficients and the two
+// projection tables (plain rows for the FFMA2 loops, pre-split mma A fragments for the tensor-core path).
+std::vector<unsigned char> build_octtabs(int NM, int M, int MT, const std::vector<double>& dird, const std::vector<float4>& lkc,
+                                         const std::vector<float>& Mt, const std::vector<float>& Dt)
+{
+    const OctTab T = octtab_layout(NM, M, MT);
+    std::vector<unsigned char> blob(8 * T.total, 0);
+    const int pitch = (NM + 3) / 4 * 4;
+    for (int oc = 0; oc < 8; ++oc) {
+        unsigned char* b = blob.data() + size_t(oc) * T.total;
+        std::memcpy(b + T.dir, dird.data() + size_t(oc) * M * 4, size_t(M) * 32);
+        std::memcpy(b + T.lk, lkc.data() + size_t(oc) * M, size_t(M) * 16);
+        auto mt = [&](int n, int lm) { return n < M ? Mt[(size_t(oc) * M + n) * NM + lm] : 0.0f; };
+        auto dt = [&](int n, int lm) { return n < M ? Dt[(size_t(oc) * M + n) * NM + lm] : 0.0f; };
+        if (MT == 0) {
+            float* m = reinterpret_cast<float*>(b + T.t0);
+            float* d = reinterpret_cast<float*>(b + T.t2);
+            for (int n = 0; n < M; ++n)
+                for (int lm = 0; lm < NM; ++lm) { m[n * pitch + lm] = mt(n, lm); d[n * pitch + lm] = dt(n, lm); }
+        } else {
+            auto put = [](float* hi, float* lo, int lane, const float v[4]) {
+                for (int r = 0; r < 4; ++r) { const float h = tf32_rna(v[r]); hi[lane * 4 + r] = h; lo[lane * 4 + r] = tf32_rna(v[r] - h); }
+            };
+            float* a0 = reinterpret_cast<float*>(b + T.t0);
+            for (int t = 0; t < MT; ++t)
+                for (int ks = 0; ks < 2; ++ks) {
+                    float* hi = a0 + size_t((t * 2 + ks) * 2 + 0) * 128;
+                    float* lo = a0 + size_t((t * 2 + ks) * 2 + 1) * 128;
+                    for (int lane = 0; lane < 32; ++lane) {
+                        const int g = lane >> 2, q = lane & 3;
+                        const float v[4] = {mt(16 * t + g, 8 * ks + q), mt(16 * t + g + 8, 8 * ks + q), mt(16 * t + g, 8 * ks + q + 4), mt(16 * t + g + 8, 8 * ks + q + 4)};
+                        put(hi, lo, lane, v);
+                    }
+                }
+            float* a2 = reinterpret_cast<float*>(b + T.t2);
+            for (int ks = 0; ks < 2 * MT; ++ks) {
+                float* hi = a2 + size_t(ks * 2 + 0) * 128;
+                float* lo = a2 + size_t(ks * 2 + 1) * 128;
+                for (int lane = 0; lane < 32; ++lane) {
+                    const int g = lane >> 2, q = lane & 3;
+                    const float v[4] = {dt(8 * ks + q, g), dt(8 * ks + q, g + 8), dt(8 * ks + q + 4, g), dt(8 * ks + q + 4, g + 8)};
+                    put(hi, lo, lane, v);
+                }
+            }
+        }
+    }
+    return blob;
+}
 
 }  // namespace
 
@@ -760,24 +819,14 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         CK(cudaMemcpyAsync(at<uint2>(p, P.o_tasks), tasks.data(), tasks.size() * sizeof(uint2), cudaMemcpyHostToDevice, st));
         CK(cudaMemsetAsync(at<unsigned>(p, P.o_flags), 0, size_t(P.chunk) * 8 * P.nbricks * 4, st));
 
-        // tensor maps over the pitched arrays (x fastest)
         {
-            // brick-major arrays: a brick's cells of one moment are tm_rows contiguous rows of tm_inner cells
-            cuuint64_t d4[4] = {cuuint64_t(P.tm_inner), cuuint64_t(P.tm_rows) * P.nbricks, cuuint64_t(NM), cuuint64_t(P.chunk)};
-            cuuint64_t s4[3] = {cuuint64_t(P.tm_inner) * 4, cuuint64_t(cp) * 4, cuuint64_t(cp) * NM * 4};
-            cuuint32_t b4[4] = {cuuint32_t(P.tm_inner), cuuint32_t(P.tm_rows), cuuint32_t(NM), 1};
-            rc = make_tensor_map(p, &SL.tmQ, at<float>(p, P.o_Q), 4, d4, s4, b4);
-            if (rc != DOCTORS_OK) return rc;
-            d4[3] = cuuint64_t(P.chunk) * G;
-            rc = make_tensor_map(p, &SL.tmPhi, at<float>(p, P.o_phiall), 4, d4, s4, b4);
-            if (rc != DOCTORS_OK) return rc;
-            cuuint64_t s2[1] = {cuuint64_t(P.tm_inner) * 8};
-            rc = make_tensor_map(p, &SL.tmSig, at<double>(p, P.o_sigt), 2, d4, s2, b4, CU_TENSOR_MAP_DATA_TYPE_FLOAT64);
-            if (rc != DOCTORS_OK) return rc;
+            const std::vector<unsigned char> blob = build_octtabs(NM, M, P.MT, dird, lkc, Mt_f, Dt_f);
+            CK(cudaMemcpyAsync(at<unsigned char>(p, P.o_octtab), blob.data(), blob.size(), cudaMemcpyHostToDevice, st));
+            CK(cudaStreamSynchronize(st));
         }
         int max_ctas = 0;
         cudaError_t e;
-        DISPATCH_NM_FIX(NM, o.closure == 1, e = (prep_brick<NM, FIX>(P.smem, 32 * P.W, &max_ctas)));
+        DISPATCH_NM_FIX(NM, o.closure == 1, P.MT, e = (prep_brick<NM, FIX, MT>(P.smem, 32 * P.W, &max_ctas)));
         if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "sweep kernel setup failed: %s (smem %zu)", cudaGetErrorString(e), P.smem);
         if (max_ctas < 1) return fail(p, DOCTORS_CUDA, "sweep kernel does not fit an SM (smem %zu)", P.smem);
         ctas_per_sm = o.ctas_per_sm > 0 ? std::min(o.ctas_per_sm, max_ctas) : max_ctas;
@@ -787,13 +836,14 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         bp.nx = nx; bp.ny = ny; bp.nz = nz;
         bp.BX = P.B[0]; bp.BY = P.B[1]; bp.BZ = P.B[2];
         bp.gbx = P.gb[0]; bp.gby = P.gb[1]; bp.gbz = P.gb[2];
-        bp.M = M; bp.W = P.W; bp.g = 0; bp.Gs = G; bp.epoch = 0; bp.tm_rows = P.tm_rows;
+        bp.M = M; bp.W = P.W; bp.g = 0; bp.Gs = G; bp.epoch = 0;
+        bp.NCb = P.NCb; bp.cells_p = P.cells_p;
+        bp.Q = at<float>(p, P.o_Q); bp.phi = at<float>(p, P.o_phiall); bp.sigt = at<double>(p, P.o_sigt);
+        bp.octtab = at<unsigned char>(p, P.o_octtab);
         bp.tasks = at<uint2>(p, P.o_tasks);
         bp.ctl = at<Control>(p, P.o_ctl);
         bp.flags = at<unsigned>(p, P.o_flags);
         bp.faceX = at<double>(p, P.o_fx); bp.faceY = at<double>(p, P.o_fy); bp.faceZ = at<double>(p, P.o_fz);
-        bp.Mtab = at<float>(p, P.o_mtab); bp.Dtab = at<float>(p, P.o_dtab);
-        bp.dird = at<double>(p, P.o_dird); bp.leakcoef = at<float4>(p, P.o_lk);
         bp.dbg_plane = nullptr;
         bp.dbg_time = nullptr;
         bp.bulk_faces = (P.face_x_n % 2 == 0 && P.face_y_n % 2 == 0 && P.face_z_n % 2 == 0) ? 1 : 0;
@@ -902,7 +952,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
                             // problems done (k_group_begin), so their tasks are skipped
                             SL.bp.ntasks = oct_begin[l + 1] - oct_begin[l];
                             cudaError_t e;
-                            DISPATCH_NM_FIX(NM, o.closure == 1, e = (launch_brick<NM, FIX>(SL, st)));
+                            DISPATCH_NM_FIX(NM, o.closure == 1, P.MT, e = (launch_brick<NM, FIX, MT>(SL, st)));
                             if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "sweep launch failed: %s", cudaGetErrorString(e));
                             ++sweep_launches; ++kernel_launches;
                         }
@@ -988,6 +1038,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         info->n_chunks = P.nchunks;
         info->brick[0] = P.B[0]; info->brick[1] = P.B[1]; info->brick[2] = P.B[2];
         info->ctas_per_sm = ctas_per_sm;
+        info->projection_mtiles = P.sweep_mode == 0 ? P.MT : 0;
     }
     for (auto e : sweep_ev) cudaEventDestroy(e);
     for (auto e : fixed_ev) cudaEventDestroy(e);
@@ -1025,51 +1076,46 @@ extern "C" int doctors_debug_device_brick_steps(doctors_problem* p, int bx, int 
         return fail(p, DOCTORS_INVALID_ARG, "brick: bx a multiple of 4 (<= 64), by * bz <= 32");
     CK(cudaSetDevice(p->device));
     const int NC = bx * by * bz;
-    const size_t smem = brick_smem_layout(1, bx, by, bz, 1).total;
-    // scratch: Q, phi (float), sigt (double), faces (double), tables, control
-    struct Scratch { float* Q; float* phi; double* sig; double* face; float* tab; double* dird; float4* lk; uint2* task;
+    const size_t smem = brick_smem_layout(1, bx, by, bz, 1, 0).total;
+    // scratch: Q, phi (float), sigt (double), faces (double), table blobs, control
+    struct Scratch { float* Q; float* phi; double* sig; double* face; unsigned char* tab; uint2* task;
                      unsigned* flags; Control* ctl; ProbState* st; double* leak; int* planes; } S;
     const size_t nface = size_t(by) * bz + size_t(bx) * bz + size_t(bx) * by;
+    const OctTab T = octtab_layout(1, 1, 0);
     char* base = nullptr;
-    const size_t bytes = 4096 + size_t(NC) * (4 + 4 + 8 + 4) + nface * 8 * 2 + 1024;
+    const size_t bytes = 8192 + size_t(NC) * (4 + 4 + 8 + 4) + nface * 8 * 2 + 8 * T.total;
     CK(cudaMalloc(&base, bytes));
     CK(cudaMemset(base, 0, bytes));
     size_t off = 0;
     auto take = [&](size_t n) { char* r = base + off; off = align_up(off + n, 256); return r; };
     S.Q = (float*)take(size_t(NC) * 4); S.phi = (float*)take(size_t(NC) * 4); S.sig = (double*)take(size_t(NC) * 8);
     S.planes = (int*)take(size_t(NC) * 4); S.face = (double*)take(nface * 8);
-    S.tab = (float*)take(64); S.dird = (double*)take(8 * 32); S.lk = (float4*)take(8 * 16); S.task = (uint2*)take(16);
+    S.tab = (unsigned char*)take(8 * T.total); S.task = (uint2*)take(16);
     S.flags = (unsigned*)take(64); S.ctl = (Control*)take(sizeof(Control)); S.st = (ProbState*)take(sizeof(ProbState)); S.leak = (double*)take(8);
     if (off > bytes) { cudaFree(base); return fail(p, DOCTORS_ALLOC, "debug scratch too small"); }
     const uint2 task = make_uint2(uint32_t(octant) << 8, 0u);
-    double dd[32]; for (int i = 0; i < 32; ++i) dd[i] = (i % 4 == 3) ? 3.0 : 1.0;
-    float one[16]; for (int i = 0; i < 16; ++i) one[i] = 1.0f;
+    {
+        // one direction per octant with coefficients (1, 1, 1, sum 3) and unit projection tables
+        std::vector<double> dd(32); for (int i = 0; i < 32; ++i) dd[i] = (i % 4 == 3) ? 3.0 : 1.0;
+        std::vector<float4> lk(8, make_float4(0.f, 0.f, 0.f, 0.f));
+        std::vector<float> one(8, 1.0f);
+        const std::vector<unsigned char> blob = build_octtabs(1, 1, 0, dd, lk, one, one);
+        cudaMemcpy(S.tab, blob.data(), blob.size(), cudaMemcpyHostToDevice);
+    }
     cudaMemcpy(S.task, &task, sizeof task, cudaMemcpyHostToDevice);
-    cudaMemcpy(S.dird, dd, sizeof dd, cudaMemcpyHostToDevice);
-    cudaMemcpy(S.tab, one, sizeof one, cudaMemcpyHostToDevice);
     SweepLaunch SL;
-    int rows = 1;
-    while ((NC / 4) % rows != 0 || NC / rows > 256) ++rows;
-    const int inner = NC / rows;
-    cuuint64_t d4[4] = {cuuint64_t(inner), cuuint64_t(rows), 1, 1};
-    cuuint64_t s4[3] = {cuuint64_t(inner) * 4, cuuint64_t(NC) * 4, cuuint64_t(NC) * 4};
-    cuuint64_t s2[1] = {cuuint64_t(inner) * 8};
-    cuuint32_t b4[4] = {cuuint32_t(inner), cuuint32_t(rows), 1, 1};
-    int rc = make_tensor_map(p, &SL.tmQ, S.Q, 4, d4, s4, b4);
-    if (rc == DOCTORS_OK) rc = make_tensor_map(p, &SL.tmPhi, S.phi, 4, d4, s4, b4);
-    if (rc == DOCTORS_OK) rc = make_tensor_map(p, &SL.tmSig, S.sig, 2, d4, s2, b4, CU_TENSOR_MAP_DATA_TYPE_FLOAT64);
-    if (rc != DOCTORS_OK) { cudaFree(base); return rc; }
     BrickParams& bp = SL.bp;
     std::memset(&bp, 0, sizeof bp);
     bp.nx = bx; bp.ny = by; bp.nz = bz; bp.BX = bx; bp.BY = by; bp.BZ = bz; bp.gbx = bp.gby = bp.gbz = 1;
-    bp.M = 1; bp.W = 1; bp.tm_rows = rows; bp.g = 0; bp.Gs = 1; bp.epoch = 1; bp.task_begin = 0; bp.ntasks = 1; bp.counter_slot = 0;
+    bp.M = 1; bp.W = 1; bp.g = 0; bp.Gs = 1; bp.epoch = 1; bp.task_begin = 0; bp.ntasks = 1; bp.counter_slot = 0;
+    bp.NCb = NC; bp.cells_p = NC; bp.Q = S.Q; bp.phi = S.phi; bp.sigt = S.sig; bp.octtab = S.tab;
     bp.tasks = S.task; bp.ctl = S.ctl; bp.flags = S.flags;
     bp.faceX = S.face; bp.faceY = S.face + size_t(by) * bz; bp.faceZ = bp.faceY + size_t(bx) * bz;
-    bp.Mtab = S.tab; bp.Dtab = S.tab; bp.dird = S.dird + 4 * 0; bp.leakcoef = S.lk; bp.state = S.st; bp.leak = S.leak;
+    bp.state = S.st; bp.leak = S.leak;
     bp.dbg_time = nullptr; bp.dbg_plane = S.planes;
-    cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<1, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+    cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<1, false, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
     if (e == cudaSuccess) {
-        k_sweep_brick<1, false, true><<<1, 32, smem, p->stream>>>(SL.tmQ, SL.tmPhi, SL.tmSig, bp);
+        k_sweep_brick<1, false, 0, true><<<1, 32, smem, p->stream>>>(bp);
         e = cudaGetLastError();
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);

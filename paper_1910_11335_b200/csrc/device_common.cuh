@@ -177,6 +177,11 @@ __device__ __forceinline__ void bulk_store(void* dst, uint32_t src, uint32_t byt
 {
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
 }
+// shared -> global elementwise fp32 add through the TMA unit (the adds happen in L2)
+__device__ __forceinline__ void bulk_reduce_add_f32(float* dst, uint32_t src, uint32_t bytes)
+{
+    asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f32 [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
+}
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
@@ -215,6 +220,40 @@ __device__ __forceinline__ void st_release_u32(unsigned* p, unsigned v)
 {
     asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
+
+// ---- tensor-core helpers for the 16-wide projections (legacy warp-level mma, TF32 operands, fp32 accumulate) ----
+// D(16x8) += A(16x8, row) * B(8x8, col).  Fragment ownership (g = lane >> 2, t = lane & 3):
+//   a0 (g, t)  a1 (g+8, t)  a2 (g, t+4)  a3 (g+8, t+4);   b0 (k = t, n = g)  b1 (k = t+4, n = g);
+//   d0 (g, 2t)  d1 (g, 2t+1)  d2 (g+8, 2t)  d3 (g+8, 2t+1).
+__device__ __forceinline__ void mma_tf32(float (&d)[4], const float4& a, float b0, float b1)
+{
+    asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+                 : "r"(__float_as_uint(a.x)), "r"(__float_as_uint(a.y)), "r"(__float_as_uint(a.z)), "r"(__float_as_uint(a.w)),
+                   "r"(__float_as_uint(b0)), "r"(__float_as_uint(b1)));
+}
+// v = hi + lo with hi exactly representable in TF32 (rounded to nearest: add half an ulp, clear 13 bits — plain
+// integer ALU; cvt.rna.tf32.f32 expands to four instructions here); lo = v - hi is exact in fp32, of either
+// sign, and is truncated to TF32 by the tensor core: |v - hi - tf32(lo)| <= 2^-21 |v|, unbiased
+__device__ __forceinline__ void split_tf32(float v, float& hi, float& lo)
+{
+    hi = __uint_as_float((__float_as_uint(v) + 0x1000u) & 0xffffe000u);
+    lo = v - hi;
+}
+__device__ __forceinline__ float4 lds_v4f32(uint32_t a)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a) : "memory");
+    return v;
+}
+// 3-product split: acc += a * b with a = (ah, al), b = (bh, bl); small terms first
+__device__ __forceinline__ void mma_3xtf32(float (&d)[4], const float4& ah, const float4& al, float bh0, float bh1, float bl0, float bl1)
+{
+    mma_tf32(d, al, bh0, bh1);
+    mma_tf32(d, ah, bl0, bl1);
+    mma_tf32(d, ah, bh0, bh1);
+}
+__device__ __forceinline__ void sts_v2f32(uint32_t a, float x, float y) { asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(a), "f"(x), "f"(y) : "memory"); }
 
 // ---- one cell, one direction: diamond difference (readings R1, R2) -----------
 //   psi = (q + cx a + cy b + cz c) / (sigt + cx + cy + cz),  out_d = 2 psi - in_d

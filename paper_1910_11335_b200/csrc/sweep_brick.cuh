@@ -14,13 +14,22 @@
 //            in a register, the y and z faces are handed to lanes (j'+1,k') / (j',k'+1) by warp
 //            shuffles: no shared-memory traffic, no block barrier inside the wavefront.
 //
-// Per task:  TMA loads Q_lm [NM][brick] (fp32) and sigma_t [brick] (fp64) into shared memory;
-// phase 0 projects moments -> directions (q_n, a5) for the whole brick; the wavefront phase applies
-// the diamond-difference update (a4) in place (q_n -> psi_n), its face recurrence in fp64;
-// brick-to-brick faces go through global buffers (L2) guarded by release/acquire flags; phase 2
-// projects directions -> moments (Eq. 3) for the whole brick and one TMA reduce-add adds the tile
-// into phi in L2 (so octants may touch a cell concurrently — the paper's obstacle at PAPER.md:119).
-// The angular flux never leaves the SM.
+// Per task:  bulk async copies (TMA unit) bring Q_lm [NM][brick] (fp32, one contiguous run per moment in
+// the brick-major layout), sigma_t [brick] (fp64) and, when the octant changes, the octant's table blob
+// into shared memory; phase 0 projects moments -> directions (q_n, a5) for the whole brick; the
+// wavefront phase applies the diamond-difference update (a4) in place (q_n -> psi_n), its face
+// recurrence in fp64; brick-to-brick faces go through global buffers (L2) guarded by release/acquire
+// flags; phase 2 projects directions -> moments (Eq. 3) for the whole brick and bulk reduce-adds
+// (cp.reduce.async.bulk .add.f32) add the tile into phi in L2 (so octants may touch a cell concurrently
+// — the paper's obstacle at PAPER.md:119).  The angular flux never leaves the SM.
+//
+// Projections (a5), template parameter MT:
+//   MT = 0  plain FFMA2 loops (any NM, any M).
+//   MT >= 1 (NM = 16, M <= 16 MT): the two 16-wide contractions run on the tensor cores as
+//           mma.sync m16n8k8 TF32 with the 3-product split (a_hi b_lo + a_lo b_hi + a_hi b_hi, fp32
+//           accumulate): per-term relative error ~2^-21, well inside the 1e-4 gate.  The
+//           coefficient tables arrive pre-split and in fragment order (host_tables / api.cu), moment planes
+//           sit at a pitch = 8 (mod 32) words so fragment loads and stores are bank-conflict free.
 #pragma once
 #include "device_common.cuh"
 
@@ -31,7 +40,12 @@ struct BrickParams {
     int BX, BY, BZ;              // brick extents (BX % 4 == 0, BY * BZ <= 32)
     int gbx, gby, gbz;           // brick grid
     int M;                       // directions per octant
-    int tm_rows;                 // TMA box rows per brick (tensor-map coordinate 1 of brick b = tm_rows * b)
+    int NCb;                     // cells per brick (= BX*BY*BZ): brick b of a per-cell array starts at b * NCb
+    long long cells_p;           // padded cell count (plane pitch of Q / phi in global memory)
+    const float* Q;              // [prob][NM][cells_p]
+    float* phi;                  // [prob * Gs + g][NM][cells_p]
+    const double* sigt;          // [cells_p], current group
+    const unsigned char* octtab; // [8] blobs of octtab_layout(...).total bytes
     int W;                       // sweep warps per CTA (blockDim.x = 32 W); warp w takes directions w, w+W, ...
     int g, Gs;                   // current group; group slots in the phi tensor map (coordinate 4 = prob*Gs + g)
     unsigned epoch;              // value that marks a brick done in this launch
@@ -43,10 +57,6 @@ struct BrickParams {
     double* faceX;               // [prob][8][gby*gbz][M][BZ][BY]
     double* faceY;               // [prob][8][gbx*gbz][M][BZ][BX]
     double* faceZ;               // [prob][8][gbx*gby][M][BY][BX]
-    const float* Mtab;           // [ndir][NM]
-    const float* Dtab;           // [ndir][NM]
-    const double* dird;          // [ndir][4] {2|mu|/dx, 2|eta|/dy, 2|xi|/dz, sum}  (fp64, exact coefficients)
-    const float4* leakcoef;      // [ndir] {w|mu|dy dz, w|eta|dx dz, w|xi|dx dy, 0}
     const ProbState* state;
     double* leak;                // [prob]
     int bulk_faces;              // 1: all three face blocks are multiples of 16 bytes -> moved by bulk async copies (TMA unit)
@@ -56,30 +66,64 @@ struct BrickParams {
 
 __host__ __device__ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+constexpr int kFragBytes = 512;   // one mma A fragment (4 x b32) for the 32 lanes of a warp
+template <int NM> __host__ __device__ constexpr int kTabPitch() { return (NM + 3) / 4 * 4; }   // table row pitch (16-byte rows)
+
+// Per-octant table blob (global memory, copied to shared memory by one bulk copy when a CTA changes octant):
+//   dir  [M][4] double  {2|mu|/dx, 2|eta|/dy, 2|xi|/dz, sum}   (fp64, exact coefficients)
+//   lk   [M] float4     {w|mu|dy dz, w|eta|dx dz, w|xi|dx dy, 0}
+//   MT = 0:  mt [M][pitch], dt [M][pitch] float  (moment -> direction, direction -> moment)
+//   MT >= 1: a0 [MT][2 k-steps][hi, lo][32 lanes] float4: A fragments of Mtab (rows = directions, K = moments)
+//            a2 [2 MT k-steps][hi, lo][32 lanes] float4: A fragments of Dtab^T (rows = moments, K = directions, zero beyond M)
+struct OctTab { size_t dir, lk, t0, t2, total; };
+__host__ __device__ inline OctTab octtab_layout(int NM, int M, int MT)
+{
+    OctTab o;
+    const size_t pitch = size_t((NM + 3) / 4 * 4);
+    o.dir = 0;
+    o.lk = size_t(M) * 32;
+    o.t0 = o.lk + size_t(M) * 16;
+    if (MT == 0) { o.t2 = o.t0 + size_t(M) * pitch * 4; o.total = o.t2 + size_t(M) * pitch * 4; }
+    else { o.t2 = o.t0 + size_t(MT) * 2 * 2 * kFragBytes; o.total = o.t2 + size_t(2 * MT) * 2 * kFragBytes; }
+    o.total = (o.total + 15) / 16 * 16;
+    return o;
+}
+
+// plane pitch (in floats) of the moment / direction tile in shared memory
+__host__ __device__ inline int plane_pitch(int NC, int MT)
+{
+    if (MT == 0) return NC;
+    return NC + (8 - NC % 32 + 32) % 32;       // = 8 (mod 32): conflict-free mma fragment loads / stores
+}
+
 struct BrickSmem {
-    size_t q, sig, psi, fx, fy, fz, dir, lk, mt, dt, misc, total;
+    size_t q, sig, psi, fx, fy, fz, tab, misc, total;
 };
 
-__host__ __device__ inline BrickSmem brick_smem_layout(int NM, int BX, int BY, int BZ, int M)
+__host__ __device__ inline BrickSmem brick_smem_layout(int NM, int BX, int BY, int BZ, int M, int MT)
 {
     BrickSmem s;
     size_t NC = size_t(BX) * BY * BZ, o = 0;
     s.misc = o;  o = align_up(o + 128, 128);   // mbarrier, task slots, reduction scratch; also the pad idle lanes may read
-    // one tile of max(NM, M) planes holds, in turn, Q_lm (TMA load), psi_n (in place, per cell) and the
-    // phi_lm contribution (in place again, TMA reduce-add source)
-    s.q = o;     o = align_up(o + size_t(NM > M ? NM : M) * NC * 4, 128);
+    // one tile of max(NM, M) planes holds, in turn, Q_lm (bulk loads), psi_n (in place, per cell) and the
+    // phi_lm contribution (in place again, bulk reduce-add source)
+    s.q = o;     o = align_up(o + size_t(NM > M ? NM : M) * plane_pitch(int(NC), MT) * 4, 128);
     s.sig = o;   o = align_up(o + NC * 8, 128);
     s.psi = s.q;
     s.fx = o;    o = align_up(o + size_t(M) * BY * BZ * 8, 8);      // fx, fy, fz contiguous (one load loop)
     s.fy = o;    o = align_up(o + size_t(M) * BX * BZ * 8, 8);
     s.fz = o;    o = align_up(o + size_t(M) * BX * BY * 8, 16);
-    s.dir = o;   o = align_up(o + size_t(M) * 32, 16);
-    s.lk = o;    o = align_up(o + size_t(M) * 16, 16);
-    s.mt = o;    o = align_up(o + size_t(M) * ((NM + 3) / 4 * 4) * 4, 16);
-    s.dt = o;    o = align_up(o + size_t(M) * ((NM + 3) / 4 * 4) * 4, 16);
+    s.tab = o;   o = align_up(o + octtab_layout(NM, M, MT).total, 16);
     o = align_up(o + 128, 16);                  // tail pad (idle lanes may read up to 10 cells past the tables' start)
     s.total = o;
     return s;
+}
+
+// m-tiles of 16 directions the tensor-core projections need; 0 = use the FFMA2 loops
+__host__ __device__ inline int projection_mtiles(int NM, int M, int NC)
+{
+    if (NM != 16 || NC % 8 != 0 || M > 48) return 0;
+    return (M + 15) / 16;
 }
 
 // Sub-sweep indexing inside a brick (Eq. 8): lane -> (j',k') of the cross section, step s -> i'.
@@ -89,29 +133,178 @@ __device__ __forceinline__ void lane_cross_section(int lane, int BY, int& jp, in
     kp = lane / BY;
 }
 constexpr int kFaceRegs = 7;
-template <int NM> __host__ __device__ constexpr int kTabPitch() { return (NM + 3) / 4 * 4; }   // table row pitch (16-byte rows)
 __device__ __forceinline__ int step_to_ip(int s, int jp, int kp) { return s - jp - kp; }
 
-template <int NM, bool FIX, bool DBG = false>
-__global__ void __launch_bounds__(32 * kMaxSweepWarps, 3)
-k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmPhi,
-              const __grid_constant__ CUtensorMap tmSig, const BrickParams P)
+// ---- a5 on the tensor cores ------------------------------------------------------------------------------
+// Both projections are [16 x K] x [K x cells] contractions with K <= 48.  One n-tile = 8 consecutive cells of the
+// brick; a warp works on two n-tiles at a time and reads every plane of those cells before it writes the result
+// over the same planes (in place).  Each (tile, k-step) pair owns an accumulator: four independent chains of
+// three dependent MMAs, issued round-robin in source order (ptxas keeps mma.sync in program order; a dependent
+// HMMA waits ~21 cycles, an independent one issues every 8 — measured on B200).
+// Kept out of line: the kernel around them is register-starved (64 registers for 3 CTAs per SM) and these
+// loops want their own allocation; the call costs a few spills per task instead of rematerialised addresses
+// in every iteration.
+struct MmaChains {
+    float acc[2][2][4];                                       // [tile][k-step]
+    __device__ __forceinline__ void clear()
+    {
+#pragma unroll
+        for (int u = 0; u < 2; ++u)
+#pragma unroll
+            for (int k = 0; k < 2; ++k) { acc[u][k][0] = 0.0f; acc[u][k][1] = 0.0f; acc[u][k][2] = 0.0f; acc[u][k][3] = 0.0f; }
+    }
+    // acc[u][k] += A_k * B_{u,k} with the 3-product TF32 split; small terms first
+    __device__ __forceinline__ void run(const float4 (&ah)[2], const float4 (&al)[2], const float (&bh)[2][4], const float (&bl)[2][4])
+    {
+#pragma unroll
+        for (int k = 0; k < 2; ++k)
+#pragma unroll
+            for (int u = 0; u < 2; ++u) mma_tf32(acc[u][k], al[k], bh[u][2 * k], bh[u][2 * k + 1]);
+#pragma unroll
+        for (int k = 0; k < 2; ++k)
+#pragma unroll
+            for (int u = 0; u < 2; ++u) mma_tf32(acc[u][k], ah[k], bl[u][2 * k], bl[u][2 * k + 1]);
+#pragma unroll
+        for (int k = 0; k < 2; ++k)
+#pragma unroll
+            for (int u = 0; u < 2; ++u) mma_tf32(acc[u][k], ah[k], bh[u][2 * k], bh[u][2 * k + 1]);
+    }
+};
+
+// moments -> directions:  q_n[cell] = sum_lm Mtab[n][lm] Q_lm[cell]   (rhs of Eq. 2 in moment form, R3)
+// `tile`: shared address of plane 0, `frag`: shared address of the a0 fragments (octtab_layout)
+template <int MT>
+__device__ __noinline__ void project_moments_to_directions_mma(uint32_t tile, uint32_t frag, int NC, int NCP, int M)
 {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const int gq = lane >> 2, tq = lane & 3;
+    const int NT = NC >> 3;
+    const uint32_t p4 = 16u * uint32_t(NCP);                  // four planes, in bytes
+    const uint32_t ld0 = tile + 4u * uint32_t(tq * NCP + gq);
+    const uint32_t st0 = tile + 4u * uint32_t(gq * NCP + 2 * tq);
+    const uint32_t fl = frag + 16u * uint32_t(lane);
+    float4 ah[2], al[2];
+    if constexpr (MT == 1) {
+#pragma unroll
+        for (int ks = 0; ks < 2; ++ks) { ah[ks] = lds_v4f32(fl + uint32_t(ks * 2 + 0) * kFragBytes); al[ks] = lds_v4f32(fl + uint32_t(ks * 2 + 1) * kFragBytes); }
+    }
+#pragma unroll 1
+    for (int t0 = 2 * warp; t0 < NT; t0 += 2 * nwarps) {
+        const bool two = t0 + 1 < NT;                          // a missing second tile recomputes the first (not stored)
+        float bh[2][4], bl[2][4];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            const uint32_t a = ld0 + 32u * uint32_t(t0 + (two ? u : 0));
+#pragma unroll
+            for (int r = 0; r < 4; ++r) split_tf32(lds_f32(a + uint32_t(r) * p4), bh[u][r], bl[u][r]);   // lm = tq + 4 r
+        }
+        float out[MT][2][4];
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt) {
+            if constexpr (MT > 1) {
+#pragma unroll
+                for (int ks = 0; ks < 2; ++ks) { ah[ks] = lds_v4f32(fl + uint32_t((mt * 2 + ks) * 2 + 0) * kFragBytes); al[ks] = lds_v4f32(fl + uint32_t((mt * 2 + ks) * 2 + 1) * kFragBytes); }
+            }
+            MmaChains C;
+            C.clear();
+            C.run(ah, al, bh, bl);
+#pragma unroll
+            for (int u = 0; u < 2; ++u)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) out[mt][u][e] = C.acc[u][0][e] + C.acc[u][1][e];
+        }
+        __syncwarp();
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            if (u == 0 || two) {
+                const uint32_t d = st0 + 32u * uint32_t(t0 + u);
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt) {
+                    const int n0 = 16 * mt + gq;
+                    if (n0 < M) sts_v2f32(d + uint32_t(4 * mt) * p4, out[mt][u][0], out[mt][u][1]);
+                    if (n0 + 8 < M) sts_v2f32(d + uint32_t(4 * mt + 2) * p4, out[mt][u][2], out[mt][u][3]);
+                }
+            }
+        }
+    }
+}
+
+// directions -> moments:  phi_lm[cell] (this octant's share) = sum_n Dtab[n][lm] psi_n[cell]   (Eq. 3)
+// K = 16 MT directions, two 8-wide k-steps per pass; the fragments are zero beyond M and those planes are not read.
+template <int MT>
+__device__ __noinline__ void project_directions_to_moments_mma(uint32_t tile, uint32_t frag, int NC, int NCP, int M)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const int gq = lane >> 2, tq = lane & 3;
+    const int NT = NC >> 3;
+    const uint32_t p4 = 16u * uint32_t(NCP);
+    const uint32_t ld0 = tile + 4u * uint32_t(tq * NCP + gq);
+    const uint32_t st0 = tile + 4u * uint32_t(gq * NCP + 2 * tq);
+    const uint32_t fl = frag + 16u * uint32_t(lane);
+    float4 ah[2], al[2];
+    if constexpr (MT == 1) {
+#pragma unroll
+        for (int ks = 0; ks < 2; ++ks) { ah[ks] = lds_v4f32(fl + uint32_t(ks * 2 + 0) * kFragBytes); al[ks] = lds_v4f32(fl + uint32_t(ks * 2 + 1) * kFragBytes); }
+    }
+#pragma unroll 1
+    for (int t0 = 2 * warp; t0 < NT; t0 += 2 * nwarps) {
+        const bool two = t0 + 1 < NT;
+        MmaChains C;
+        C.clear();
+#pragma unroll
+        for (int kp = 0; kp < MT; ++kp) {                     // pass kp: directions 16 kp .. 16 kp + 15
+            if (16 * kp < M) {                                // uniform
+                if constexpr (MT > 1) {
+#pragma unroll
+                    for (int ks = 0; ks < 2; ++ks) { ah[ks] = lds_v4f32(fl + uint32_t((kp * 2 + ks) * 2 + 0) * kFragBytes); al[ks] = lds_v4f32(fl + uint32_t((kp * 2 + ks) * 2 + 1) * kFragBytes); }
+                }
+                float bh[2][4], bl[2][4];
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    const uint32_t a = ld0 + 32u * uint32_t(t0 + (two ? u : 0)) + uint32_t(4 * kp) * p4;
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) {             // direction n = 16 kp + tq + 4 r  (k-step r / 2)
+                        const float v = 16 * kp + tq + 4 * r < M ? lds_f32(a + uint32_t(r) * p4) : 0.0f;
+                        split_tf32(v, bh[u][r], bl[u][r]);
+                    }
+                }
+                C.run(ah, al, bh, bl);
+            }
+        }
+        __syncwarp();
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            if (u == 0 || two) {
+                const uint32_t d = st0 + 32u * uint32_t(t0 + u);
+                sts_v2f32(d, C.acc[u][0][0] + C.acc[u][1][0], C.acc[u][0][1] + C.acc[u][1][1]);
+                sts_v2f32(d + 2u * p4, C.acc[u][0][2] + C.acc[u][1][2], C.acc[u][0][3] + C.acc[u][1][3]);
+            }
+        }
+    }
+}
+
+template <int NM, bool FIX, int MT, bool DBG = false>
+__global__ void __launch_bounds__(32 * kMaxSweepWarps, 3)
+k_sweep_brick(const BrickParams P)
+{
+    static_assert(MT == 0 || NM == 16, "tensor-core projections are written for P3 (16 moments)");
     if (__ldcg(&P.ctl->all_done)) return;                              // every problem of the chunk has stopped (a6): nothing to sweep
     extern __shared__ __align__(128) unsigned char smem[];
     const int BX = P.BX, BY = P.BY, BZ = P.BZ, M = P.M;
     const int NC = BX * BY * BZ;
-    const BrickSmem L = brick_smem_layout(NM, BX, BY, BZ, M);
+    const int NCP = plane_pitch(NC, MT);                              // plane pitch of the tile (floats)
+    const BrickSmem L = brick_smem_layout(NM, BX, BY, BZ, M, MT);
+    const OctTab T = octtab_layout(NM, M, MT);
     float* sQ = reinterpret_cast<float*>(smem + L.q);
     double* sSig = reinterpret_cast<double*>(smem + L.sig);
     float* sPsi = reinterpret_cast<float*>(smem + L.psi);
     double* sFx = reinterpret_cast<double*>(smem + L.fx);
     double* sFy = reinterpret_cast<double*>(smem + L.fy);
     double* sFz = reinterpret_cast<double*>(smem + L.fz);
-    double* sDir = reinterpret_cast<double*>(smem + L.dir);          // [M][4]
-    float4* sLk = reinterpret_cast<float4*>(smem + L.lk);
-    float* sM = reinterpret_cast<float*>(smem + L.mt);
-    float* sD = reinterpret_cast<float*>(smem + L.dt);
+    double* sDir = reinterpret_cast<double*>(smem + L.tab + T.dir);  // [M][4]
+    float4* sLk = reinterpret_cast<float4*>(smem + L.tab + T.lk);
+    float* sM = reinterpret_cast<float*>(smem + L.tab + T.t0);      // MT = 0: [M][pitch];  MT >= 1: A fragments (float4 per lane)
+    float* sD = reinterpret_cast<float*>(smem + L.tab + T.t2);
     uint64_t* sBar = reinterpret_cast<uint64_t*>(smem + L.misc);
     int* sTask = reinterpret_cast<int*>(smem + L.misc + 8);
     float* sRed = reinterpret_cast<float*>(smem + L.misc + 64);     // kMaxSweepWarps floats
@@ -169,27 +362,19 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         double* gFy = P.faceY + (po * (P.gbx * P.gbz) + bi + P.gbx * bk) * (size_t)faceYn;
         double* gFz = P.faceZ + (po * (P.gbx * P.gby) + bi + P.gbx * bj) * (size_t)faceZn;
 
-        // octant tables (directions of this octant are contiguous: n = oct*M + m): loaded by warps 1.. while
-        // warp 0 issues the tile load and polls the flags, so that their global-load latency is hidden
-        if (oct != last_oct) {
-            const int tt = nthr > 32 ? tid - 32 : tid, tn = nthr > 32 ? nthr - 32 : nthr;
-            if (tt >= 0) {
-                for (int e = tt; e < M * NM; e += tn) {
-                    const int n = e / NM, lm = e - n * NM;
-                    sM[n * kTabPitch<NM>() + lm] = P.Mtab[(size_t)oct * M * NM + e];
-                    sD[n * kTabPitch<NM>() + lm] = P.Dtab[(size_t)oct * M * NM + e];
-                }
-                for (int e = tt; e < M * 4; e += tn) sDir[e] = P.dird[(size_t)oct * M * 4 + e];
-                for (int e = tt; e < M; e += tn) sLk[e] = P.leakcoef[oct * M + e];
-            }
-            last_oct = oct;
-        }
+        // tile, sigma_t and (when the octant changes) the octant's table blob: bulk async copies, one mbarrier.
+        // Directions of an octant are contiguous (n = oct*M + m); nobody reads the old tables any more (end-of-task barrier).
         if (tid == 0) {
-            bulk_wait_read0();                                   // previous tile's reduce has read sQ
-            mbar_expect_tx(bar, uint32_t(NM * NC * 4 + NC * 8));
-            tma_load_4d(smem_u32(sQ), &tmQ, bar, 0, P.tm_rows * brick, 0, prob);
-            tma_load_2d(smem_u32(sSig), &tmSig, bar, 0, P.tm_rows * brick);
+            bulk_wait_read0();                                   // previous tile's reduce-adds have read sQ
+            const bool tab = oct != last_oct;
+            mbar_expect_tx(bar, uint32_t(NM * NC * 4 + NC * 8 + (tab ? T.total : 0)));
+            const float* gq = P.Q + (size_t)prob * NM * P.cells_p + (size_t)brick * P.NCb;
+#pragma unroll 1
+            for (int lm = 0; lm < NM; ++lm) bulk_load(smem_u32(sQ + lm * NCP), gq + (size_t)lm * P.cells_p, uint32_t(NC * 4), bar);
+            bulk_load(smem_u32(sSig), P.sigt + (size_t)brick * P.NCb, uint32_t(NC * 8), bar);
+            if (tab) bulk_load(smem_u32(smem + L.tab), P.octtab + (size_t)oct * T.total, uint32_t(T.total), bar);
         }
+        last_oct = oct;
         TICK(9);
         // wait for the upwind bricks of this (problem, octant): one warp-0 lane per upwind flag
         if (warp == 0) {
@@ -242,36 +427,40 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         TICK(3);
 
         // ---- phase 0: q_n = sum_lm Mtab[n][lm] Q_lm for every cell of the brick (a5) ----
-        // Two cells per thread share every coefficient load (the phase is bound by the shared-memory pipe);
-        // packed fp32x2 FMAs (FFMA2, sm_100) accumulate even / odd moments in the halves of a register pair.
-        for (int c = tid; c < NC; c += 2 * nthr) {
-            const int c2 = c + nthr;
-            const bool two = c2 < NC;
-            if constexpr (NM >= 2) {
-                float2 qa[NM / 2], qb[NM / 2];
-#pragma unroll
-                for (int k = 0; k < NM / 2; ++k) {
-                    qa[k] = make_float2(sQ[(2 * k) * NC + c], sQ[(2 * k + 1) * NC + c]);
-                    qb[k] = two ? make_float2(sQ[(2 * k) * NC + c2], sQ[(2 * k + 1) * NC + c2]) : make_float2(0.0f, 0.0f);
-                }
-                float qla = 0.0f, qlb = 0.0f;
-                if (NM & 1) { qla = sQ[(NM - 1) * NC + c]; qlb = two ? sQ[(NM - 1) * NC + c2] : 0.0f; }
-                for (int n = 0; n < M; ++n) {
-                    const float2* mt = reinterpret_cast<const float2*>(sM + n * kTabPitch<NM>());
-                    float2 a = make_float2(0.0f, 0.0f), b = make_float2(0.0f, 0.0f);
-#pragma unroll
-                    for (int k = 0; k < NM / 2; ++k) { const float2 m2 = mt[k]; a = __ffma2_rn(m2, qa[k], a); b = __ffma2_rn(m2, qb[k], b); }
-                    float ra = a.x + a.y, rb = b.x + b.y;
-                    if (NM & 1) { const float ml = sM[n * kTabPitch<NM>() + NM - 1]; ra = fmaf(ml, qla, ra); rb = fmaf(ml, qlb, rb); }
-                    sPsi[n * NC + c] = ra;                       // in place: this thread has read all of its cells
-                    if (two) sPsi[n * NC + c2] = rb;
-                }
-            } else {
-                const float qa0 = sQ[c], qb0 = two ? sQ[c2] : 0.0f;
-                for (int n = 0; n < M; ++n) {
-                    const float m0 = sM[n * kTabPitch<NM>()];
-                    sPsi[n * NC + c] = m0 * qa0;
-                    if (two) sPsi[n * NC + c2] = m0 * qb0;
+        if constexpr (MT >= 1) {
+            project_moments_to_directions_mma<MT>(smem_u32(sQ), smem_u32(sM), NC, NCP, M);
+        } else {
+            // Two cells per thread share every coefficient load (the phase is bound by the shared-memory pipe);
+            // packed fp32x2 FMAs (FFMA2, sm_100) accumulate even / odd moments in the halves of a register pair.
+            for (int c = tid; c < NC; c += 2 * nthr) {
+                const int c2 = c + nthr;
+                const bool two = c2 < NC;
+                if constexpr (NM >= 2) {
+                    float2 qa[NM / 2], qb[NM / 2];
+    #pragma unroll
+                    for (int k = 0; k < NM / 2; ++k) {
+                        qa[k] = make_float2(sQ[(2 * k) * NCP + c], sQ[(2 * k + 1) * NCP + c]);
+                        qb[k] = two ? make_float2(sQ[(2 * k) * NCP + c2], sQ[(2 * k + 1) * NCP + c2]) : make_float2(0.0f, 0.0f);
+                    }
+                    float qla = 0.0f, qlb = 0.0f;
+                    if (NM & 1) { qla = sQ[(NM - 1) * NCP + c]; qlb = two ? sQ[(NM - 1) * NCP + c2] : 0.0f; }
+                    for (int n = 0; n < M; ++n) {
+                        const float2* mt = reinterpret_cast<const float2*>(sM + n * kTabPitch<NM>());
+                        float2 a = make_float2(0.0f, 0.0f), b = make_float2(0.0f, 0.0f);
+    #pragma unroll
+                        for (int k = 0; k < NM / 2; ++k) { const float2 m2 = mt[k]; a = __ffma2_rn(m2, qa[k], a); b = __ffma2_rn(m2, qb[k], b); }
+                        float ra = a.x + a.y, rb = b.x + b.y;
+                        if (NM & 1) { const float ml = sM[n * kTabPitch<NM>() + NM - 1]; ra = fmaf(ml, qla, ra); rb = fmaf(ml, qlb, rb); }
+                        sPsi[n * NCP + c] = ra;                       // in place: this thread has read all of its cells
+                        if (two) sPsi[n * NCP + c2] = rb;
+                    }
+                } else {
+                    const float qa0 = sQ[c], qb0 = two ? sQ[c2] : 0.0f;
+                    for (int n = 0; n < M; ++n) {
+                        const float m0 = sM[n * kTabPitch<NM>()];
+                        sPsi[n * NCP + c] = m0 * qa0;
+                        if (two) sPsi[n * NCP + c2] = m0 * qb0;
+                    }
                 }
             }
         }
@@ -307,7 +496,7 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
             const double cx = sDir[4 * n], cy = sDir[4 * n + 1], cz = sDir[4 * n + 2], cs = sDir[4 * n + 3];
             double* fxp = sFx + n * (BY * BZ) + lj + BY * lk_;
             // running shared-memory addresses of this lane's cell: advanced by one cell (sx) per step
-            uint32_t pq = smem_u32(sPsi) + (lane_ok ? 4u * (uint32_t(n * NC) + row) : 0u);
+            uint32_t pq = smem_u32(sPsi) + (lane_ok ? 4u * (uint32_t(n * NCP) + row) : 0u);
             uint32_t ps = smem_u32(sSig) + (lane_ok ? 8u * row : 0u);
             uint32_t py = smem_u32(sFy) + (lane_ok ? 8u * uint32_t((n * BZ + lk_) * BX + li0) : 0u);
             uint32_t pz = smem_u32(sFz) + (lane_ok ? 8u * uint32_t((n * BY + lj) * BX + li0) : 0u);
@@ -328,7 +517,7 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
                 sts_f64_if(act && last_y, py, oy);
                 sts_f64_if(act && last_z, pz, oz);
                 if (act) ax = ox;
-                if (DBG && act) P.dbg_plane[(pq - smem_u32(sPsi)) / 4u - uint32_t(n * NC)] = nsteps - s;
+                if (DBG && act) P.dbg_plane[(pq - smem_u32(sPsi)) / 4u - uint32_t(n * NCP)] = nsteps - s;
                 ++ip; pq += d4; ps += d8; py += d8; pz += d8;
             }
             if (lane_ok) *fxp = ax;
@@ -375,38 +564,42 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         }
         TICK(6);
 
-        // ---- phase 2: phi_lm += sum_n Dtab[n][lm] psi_n (Eq. 3, a5), tile -> sQ, TMA reduce-add ----
-        for (int c = tid; c < NC; c += 2 * nthr) {
-            const int c2 = c + nthr;
-            const bool two = c2 < NC;
-            if constexpr (NM >= 2) {
-                float2 pa[NM / 2], pb[NM / 2];
-                float pla = 0.0f, plb = 0.0f;
-#pragma unroll
-                for (int k = 0; k < NM / 2; ++k) { pa[k] = make_float2(0.0f, 0.0f); pb[k] = make_float2(0.0f, 0.0f); }
-                for (int n = 0; n < M; ++n) {
-                    const float2* dt = reinterpret_cast<const float2*>(sD + n * kTabPitch<NM>());
-                    const float va = sPsi[n * NC + c], vb = two ? sPsi[n * NC + c2] : 0.0f;
-                    const float2 va2 = make_float2(va, va), vb2 = make_float2(vb, vb);
-#pragma unroll
-                    for (int k = 0; k < NM / 2; ++k) { const float2 d2 = dt[k]; pa[k] = __ffma2_rn(d2, va2, pa[k]); pb[k] = __ffma2_rn(d2, vb2, pb[k]); }
-                    if (NM & 1) { const float dl = sD[n * kTabPitch<NM>() + NM - 1]; pla = fmaf(dl, va, pla); plb = fmaf(dl, vb, plb); }
+        // ---- phase 2: phi_lm += sum_n Dtab[n][lm] psi_n (Eq. 3, a5), tile -> sQ, bulk reduce-adds ----
+        if constexpr (MT >= 1) {
+            project_directions_to_moments_mma<MT>(smem_u32(sQ), smem_u32(sD), NC, NCP, M);
+        } else {
+            for (int c = tid; c < NC; c += 2 * nthr) {
+                const int c2 = c + nthr;
+                const bool two = c2 < NC;
+                if constexpr (NM >= 2) {
+                    float2 pa[NM / 2], pb[NM / 2];
+                    float pla = 0.0f, plb = 0.0f;
+    #pragma unroll
+                    for (int k = 0; k < NM / 2; ++k) { pa[k] = make_float2(0.0f, 0.0f); pb[k] = make_float2(0.0f, 0.0f); }
+                    for (int n = 0; n < M; ++n) {
+                        const float2* dt = reinterpret_cast<const float2*>(sD + n * kTabPitch<NM>());
+                        const float va = sPsi[n * NCP + c], vb = two ? sPsi[n * NCP + c2] : 0.0f;
+                        const float2 va2 = make_float2(va, va), vb2 = make_float2(vb, vb);
+    #pragma unroll
+                        for (int k = 0; k < NM / 2; ++k) { const float2 d2 = dt[k]; pa[k] = __ffma2_rn(d2, va2, pa[k]); pb[k] = __ffma2_rn(d2, vb2, pb[k]); }
+                        if (NM & 1) { const float dl = sD[n * kTabPitch<NM>() + NM - 1]; pla = fmaf(dl, va, pla); plb = fmaf(dl, vb, plb); }
+                    }
+    #pragma unroll
+                    for (int k = 0; k < NM / 2; ++k) {
+                        sQ[(2 * k) * NCP + c] = pa[k].x; sQ[(2 * k + 1) * NCP + c] = pa[k].y;
+                        if (two) { sQ[(2 * k) * NCP + c2] = pb[k].x; sQ[(2 * k + 1) * NCP + c2] = pb[k].y; }
+                    }
+                    if (NM & 1) { sQ[(NM - 1) * NCP + c] = pla; if (two) sQ[(NM - 1) * NCP + c2] = plb; }
+                } else {
+                    float pa0 = 0.0f, pb0 = 0.0f;
+                    for (int n = 0; n < M; ++n) {
+                        const float d0 = sD[n * kTabPitch<NM>()];
+                        pa0 = fmaf(d0, sPsi[n * NCP + c], pa0);
+                        if (two) pb0 = fmaf(d0, sPsi[n * NCP + c2], pb0);
+                    }
+                    sQ[c] = pa0;
+                    if (two) sQ[c2] = pb0;
                 }
-#pragma unroll
-                for (int k = 0; k < NM / 2; ++k) {
-                    sQ[(2 * k) * NC + c] = pa[k].x; sQ[(2 * k + 1) * NC + c] = pa[k].y;
-                    if (two) { sQ[(2 * k) * NC + c2] = pb[k].x; sQ[(2 * k + 1) * NC + c2] = pb[k].y; }
-                }
-                if (NM & 1) { sQ[(NM - 1) * NC + c] = pla; if (two) sQ[(NM - 1) * NC + c2] = plb; }
-            } else {
-                float pa0 = 0.0f, pb0 = 0.0f;
-                for (int n = 0; n < M; ++n) {
-                    const float d0 = sD[n * kTabPitch<NM>()];
-                    pa0 = fmaf(d0, sPsi[n * NC + c], pa0);
-                    if (two) pb0 = fmaf(d0, sPsi[n * NC + c2], pb0);
-                }
-                sQ[c] = pa0;
-                if (two) sQ[c2] = pb0;
             }
         }
         fence_proxy_async_smem();
@@ -418,7 +611,9 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
             st_release_u32(flag_base + brick, P.epoch);
         }
         if (tid == 0) {
-            tma_reduce_add_4d(&tmPhi, smem_u32(sQ), 0, P.tm_rows * brick, 0, prob * P.Gs + P.g);
+            float* gphi = P.phi + (size_t)(prob * P.Gs + P.g) * NM * P.cells_p + (size_t)brick * P.NCb;
+#pragma unroll 1
+            for (int lm = 0; lm < NM; ++lm) bulk_reduce_add_f32(gphi + (size_t)lm * P.cells_p, smem_u32(sQ + lm * NCP), uint32_t(NC * 4));
             bulk_commit();
             if (edge_x | edge_y | edge_z) {
                 float s = 0.0f;

@@ -109,6 +109,28 @@ def test_orders(pkg, orc, L, sn):
     assert worst < TOL, worst
 
 
+@pytest.mark.parametrize("sn,mtiles", [(4, 1), (8, 1), (12, 2), (16, 3)])
+@pytest.mark.parametrize("brick", [None, (4, 8, 4), (8, 3, 5)])
+def test_projection_paths_p3(pkg, orc, sn, mtiles, brick):
+    """P3 projections on the tensor cores (mma TF32, 3-product split; 1, 2, 3 m-tiles of 16 directions)
+    and in the fp32 FMA loops: both inside the gate, and within 2e-5 of each other on every moment."""
+    wl = tiny_p3_case(nx=13, ny=9, nz=6, G=2, sn=sn, L=3, seed=5)
+    ref = orc.solve(wl, closure=1)
+    shape = (wl.nz, wl.ny, wl.nx)
+    got = {}
+    for proj in (0, 1):
+        p, info = run_gpu(wl, closure=1, fixed_iters=ref["iters"], brick=brick, projection=proj)
+        ncb = info["brick"][0] * info["brick"][1] * info["brick"][2]
+        assert info["projection_mtiles"] == (mtiles if proj == 0 and ncb % 8 == 0 else 0)
+        got[proj] = np.stack([p.get_flux_moments(0, g, 3) for g in range(wl.G)])
+        p.close()
+        for g in range(wl.G):
+            e, _ = masked_rel_err(got[proj][g, 0], ref["phi"][0, g, 0].reshape(shape))
+            assert e < TOL, (proj, g, e)
+    scale = np.abs(got[1][:, 0]).max()
+    assert np.abs(got[0] - got[1]).max() / scale < 2e-5
+
+
 def test_degenerate_meshes(pkg, orc):
     for dims in [(1, 1, 1), (1, 7, 3), (5, 1, 1), (17, 2, 1)]:
         wl = tiny_p3_case(nx=dims[0], ny=dims[1], nz=dims[2], G=2, sn=4, L=1, seed=3)
