@@ -288,6 +288,7 @@ __global__ void __launch_bounds__(32 * kMaxSweepWarps, 3)
 k_sweep_brick(const BrickParams P)
 {
     static_assert(MT == 0 || NM == 16, "tensor-core projections are written for P3 (16 moments)");
+    static_assert(NM <= 16, "one tile-warp lane per moment plane, lanes 16 / 17 for sigma_t and the tables");
     if (__ldcg(&P.ctl->all_done)) return;                              // every problem of the chunk has stopped (a6): nothing to sweep
     extern __shared__ __align__(128) unsigned char smem[];
     const int BX = P.BX, BY = P.BY, BZ = P.BZ, M = P.M;
@@ -316,7 +317,7 @@ k_sweep_brick(const BrickParams P)
     lane_cross_section(lane, BY, jp, kp);
 
     const uint32_t barF = bar + 32;                                  // faces (bulk copies) complete here
-    if (tid == 0) { mbar_init(bar, 1); mbar_init(barF, 1); fence_mbar_init(); }
+    if (tid == 0) { mbar_init(bar, 1); mbar_init(barF, P.bulk_faces ? 3 : 1); fence_mbar_init(); }
     __syncthreads();
     uint32_t parity = 0;
     const int faceXn = M * BY * BZ, faceYn = M * BX * BZ, faceZn = M * BX * BY;
@@ -329,22 +330,55 @@ k_sweep_brick(const BrickParams P)
 #define TICK(i) do { } while (0)
 #endif
 
-    // The id of the next task is fetched one task ahead (the atomic's round trip hides behind the
-    // sweep).  Holding one unstarted task cannot deadlock: a CTA's held task has a higher index than
-    // its running one, so the lowest unfinished task of the whole grid is always running.
-    if (tid == 0) sTask[0] = int(atomicAdd(&P.ctl->counters[P.counter_slot], 1u));
+    // Roles inside the CTA (all of them also sweep):
+    //   tile warp   lanes 0..NM-1 own one moment plane each: bulk load of Q_lm at the start of a task, bulk reduce-add of
+    //               the phi_lm contribution at its end (same lane = same bulk group, so the lane can wait for "read done")
+    //   pollers     warp 0, lanes 0..2: wait for the upwind brick in x / y / z and issue that face's bulk load themselves
+    //   prefetcher  one thread fetches the NEXT task (id from the atomic counter, descriptor, done flag of its problem)
+    //               into shared memory while the current one runs: three dependent global round trips off the critical path.
+    //               Holding one unstarted task cannot deadlock: a CTA's held task has a higher index than its running one,
+    //               so the lowest unfinished task of the whole grid is always running.
+    //   publisher   last lane of the last warp: bulk-stores the outflow faces, and at the next loop top waits for them and
+    //               releases the brick's flag AFTER arriving at the block barrier (split barrier: nobody waits for it)
+    const int nwarps = nthr >> 5;
+    const int tileWarp = nwarps > 1 ? 1 : 0;
+    const int pfThread = nwarps > 2 ? 64 : 32 * tileWarp + 8;
+    const int pubWarp = nwarps - 1;
+    uint2* sDesc = reinterpret_cast<uint2*>(smem + L.misc + 16);   // [2]
+    int* sDone = reinterpret_cast<int*>(smem + L.misc + 104);      // [2]
+    auto fetch_task = [&](int sl) {
+        const int id = int(atomicAdd(&P.ctl->counters[P.counter_slot], 1u));
+        uint2 d = make_uint2(0u, 0u);
+        int dn = 0;
+        if (id < P.ntasks) { d = P.tasks[P.task_begin + id]; dn = __ldcg(&P.state[d.x & 0xff].done); }
+        sDesc[sl] = d; sDone[sl] = dn; sTask[sl] = id;
+    };
+    if (tid == 0) fetch_task(0);
     int slot = 0;
+    bool publish = false;                                        // publishing warp: a brick waits to be published
+    unsigned* pub_flag = nullptr;
     while (true) {
-        __syncthreads();
+        if (publish && lane == 31) bulk_wait_read0();            // the face blocks have been read out of sFx..sFz
+        bar_sync1(nthr);
+        if (publish) {
+            // the other 31 lanes run ahead to the tile wait of the next task; this one joins them there
+            if (lane == 31) {
+                bulk_wait0();                                    // the face blocks are in global memory
+                fence_proxy_async_all();
+                st_release_u32(pub_flag, P.epoch);
+            }
+            publish = false;
+        }
         const int t = sTask[slot];
         if (t >= P.ntasks) break;
-        if (tid == 32 % nthr) sTask[slot ^ 1] = int(atomicAdd(&P.ctl->counters[P.counter_slot], 1u));
+        const uint2 td = sDesc[slot];
+        const int prob_done = sDone[slot];
+        if (tid == pfThread) fetch_task(slot ^ 1);
         slot ^= 1;
         TICK(0);
-        const uint2 td = P.tasks[P.task_begin + t];
+        if (prob_done) continue;                                 // this problem has stopped (a6)
         const int prob = td.x & 0xff, oct = (td.x >> 8) & 7;
         const int bi = td.y & 0x3ff, bj = (td.y >> 10) & 0x3ff, bk = (td.y >> 20) & 0x3ff;
-        if (__ldcg(&P.state[prob].done)) { __syncthreads(); continue; }
 
         const int x0 = bi * BX, y0 = bj * BY, z0 = bk * BZ;
         const int ex = min(BX, P.nx - x0), ey = min(BY, P.ny - y0), ez = min(BZ, P.nz - z0);   // clipped extents
@@ -363,45 +397,56 @@ k_sweep_brick(const BrickParams P)
         double* gFz = P.faceZ + (po * (P.gbx * P.gby) + bi + P.gbx * bj) * (size_t)faceZn;
 
         // tile, sigma_t and (when the octant changes) the octant's table blob: bulk async copies, one mbarrier.
-        // Directions of an octant are contiguous (n = oct*M + m); nobody reads the old tables any more (end-of-task barrier).
-        if (tid == 0) {
-            bulk_wait_read0();                                   // previous tile's reduce-adds have read sQ
+        // Directions of an octant are contiguous (n = oct*M + m); nobody reads the old tables any more (loop-top barrier).
+        if (warp == tileWarp) {
             const bool tab = oct != last_oct;
-            mbar_expect_tx(bar, uint32_t(NM * NC * 4 + NC * 8 + (tab ? T.total : 0)));
+            if (lane == 0) mbar_expect_tx(bar, uint32_t(NM * NC * 4 + NC * 8 + (tab ? T.total : 0)));
             const float* gq = P.Q + (size_t)prob * NM * P.cells_p + (size_t)brick * P.NCb;
-#pragma unroll 1
-            for (int lm = 0; lm < NM; ++lm) bulk_load(smem_u32(sQ + lm * NCP), gq + (size_t)lm * P.cells_p, uint32_t(NC * 4), bar);
-            bulk_load(smem_u32(sSig), P.sigt + (size_t)brick * P.NCb, uint32_t(NC * 8), bar);
-            if (tab) bulk_load(smem_u32(smem + L.tab), P.octtab + (size_t)oct * T.total, uint32_t(T.total), bar);
+            if (lane < NM) {
+                bulk_wait_read0();                               // this lane's reduce-add of the previous task has read its plane
+                bulk_load(smem_u32(sQ + lane * NCP), gq + (size_t)lane * P.cells_p, uint32_t(NC * 4), bar);
+            }
+            if (lane == 16) bulk_load(smem_u32(sSig), P.sigt + (size_t)brick * P.NCb, uint32_t(NC * 8), bar);
+            if (tab && lane == 17) bulk_load(smem_u32(smem + L.tab), P.octtab + (size_t)oct * T.total, uint32_t(T.total), bar);
         }
         last_oct = oct;
         TICK(9);
         // wait for the upwind bricks of this (problem, octant): one warp-0 lane per upwind flag
-        if (warp == 0) {
-            const bool need = lane == 0 ? upx : (lane == 1 ? upy : (lane == 2 && upz));
-            const int up = lane == 0 ? brick - sx : (lane == 1 ? brick - sy * P.gbx : brick - sz * P.gbx * P.gby);
-            bool ready = !need;
-            while (!__all_sync(0xffffffffu, ready)) {
-                if (!ready) ready = ld_acquire_u32(flag_base + up) == P.epoch;
+        if (P.bulk_faces) {
+            if (warp == 0 && lane < 3) {
+                const bool need = lane == 0 ? upx : (lane == 1 ? upy : upz);
+                if (need) {
+                    const int up = lane == 0 ? brick - sx : (lane == 1 ? brick - sy * P.gbx : brick - sz * P.gbx * P.gby);
+                    const double* src = lane == 0 ? gFx : (lane == 1 ? gFy : gFz);
+                    const uint32_t dst = smem_u32(lane == 0 ? sFx : (lane == 1 ? sFy : sFz));
+                    const uint32_t bytes = 8u * uint32_t(lane == 0 ? faceXn : (lane == 1 ? faceYn : faceZn));
+                    while (ld_acquire_u32(flag_base + up) != P.epoch) { }
+                    fence_proxy_async_all();                     // flag acquired (generic proxy) -> async-proxy read of the face
+                    mbar_expect_tx(barF, bytes);
+                    bulk_load(dst, src, bytes, barF);            // 1-D bulk copy (TMA unit); needed after phase 0
+                } else {
+                    mbar_arrive(barF);
+                }
             }
+        } else {
+            if (warp == 0) {
+                const bool need = lane == 0 ? upx : (lane == 1 ? upy : (lane == 2 && upz));
+                const int up = lane == 0 ? brick - sx : (lane == 1 ? brick - sy * P.gbx : brick - sz * P.gbx * P.gby);
+                bool ready = !need;
+                while (!__all_sync(0xffffffffu, ready)) {
+                    if (!ready) ready = ld_acquire_u32(flag_base + up) == P.epoch;
+                }
+            }
+            __syncthreads();                                     // flags seen by warp 0 -> everyone may read faces
         }
         TICK(10);
-        __syncthreads();                                         // flags seen by thread 0 -> everyone may read faces
         TICK(1);
 
         // inflow faces: upwind brick's outflow, or vacuum.  sFx, sFy, sFz are contiguous.
         const int nxy = faceXn + faceYn, nall = nxy + faceZn;
         double fv[kFaceRegs];
         if (P.bulk_faces) {
-            // one thread hands the three blocks to the TMA unit (1-D bulk copies, complete on barF);
-            // vacuum faces are zero-filled by the threads.  Nothing here waits: the data is needed after phase 0.
-            if (tid == 0) {
-                fence_proxy_async_all();                         // flags acquired (generic proxy) -> async-proxy reads
-                mbar_expect_tx(barF, uint32_t(8 * ((upx ? faceXn : 0) + (upy ? faceYn : 0) + (upz ? faceZn : 0))));
-                if (upx) bulk_load(smem_u32(sFx), gFx, uint32_t(8 * faceXn), barF);
-                if (upy) bulk_load(smem_u32(sFy), gFy, uint32_t(8 * faceYn), barF);
-                if (upz) bulk_load(smem_u32(sFz), gFz, uint32_t(8 * faceZn), barF);
-            }
+            // vacuum faces are zero-filled by the threads; the others arrive by the pollers' bulk copies
             if (!upx) for (int e = tid; e < faceXn; e += nthr) sFx[e] = 0.0;
             if (!upy) for (int e = tid; e < faceYn; e += nthr) sFy[e] = 0.0;
             if (!upz) for (int e = tid; e < faceZn; e += nthr) sFz[e] = 0.0;
@@ -549,7 +594,7 @@ k_sweep_brick(const BrickParams P)
         if (P.bulk_faces) {
             fence_proxy_async_smem();                            // lanes' face writes -> visible to the async proxy
             __syncthreads();
-            if (tid == nthr - 1) {
+            if (warp == pubWarp && lane == 31) {
                 if (dnx) bulk_store(gFx, smem_u32(sFx), uint32_t(8 * faceXn));
                 if (dny) bulk_store(gFy, smem_u32(sFy), uint32_t(8 * faceYn));
                 if (dnz) bulk_store(gFz, smem_u32(sFz), uint32_t(8 * faceZn));
@@ -605,24 +650,22 @@ k_sweep_brick(const BrickParams P)
         fence_proxy_async_smem();
         __syncthreads();
         TICK(7);
-        if (P.bulk_faces && tid == nthr - 1) {                   // publish the brick; the others already start the next task
-            bulk_wait0();                                        // face blocks are in global memory (and read out of sFx..sFz)
-            fence_proxy_async_all();
-            st_release_u32(flag_base + brick, P.epoch);
-        }
-        if (tid == 0) {
+        if (warp == tileWarp && lane < NM) {
             float* gphi = P.phi + (size_t)(prob * P.Gs + P.g) * NM * P.cells_p + (size_t)brick * P.NCb;
-#pragma unroll 1
-            for (int lm = 0; lm < NM; ++lm) bulk_reduce_add_f32(gphi + (size_t)lm * P.cells_p, smem_u32(sQ + lm * NCP), uint32_t(NC * 4));
+            bulk_reduce_add_f32(gphi + (size_t)lane * P.cells_p, smem_u32(sQ + lane * NCP), uint32_t(NC * 4));
             bulk_commit();
-            if (edge_x | edge_y | edge_z) {
-                float s = 0.0f;
-                for (int w = 0; w < P.W; ++w) s += sRed[w];
-                atomicAdd(P.leak + prob, (double)s);
-            }
+        }
+        if (tid == 0 && (edge_x | edge_y | edge_z)) {
+            float s = 0.0f;
+            for (int w = 0; w < P.W; ++w) s += sRed[w];
+            atomicAdd(P.leak + prob, (double)s);
+        }
+        if (P.bulk_faces && warp == pubWarp) {                   // published at the loop top, after arriving at the barrier
+            publish = true;
+            pub_flag = flag_base + brick;
         }
     }
-    if (tid == 0) bulk_wait0();
+    if (warp == tileWarp) bulk_wait0();
 #ifdef DOCTORS_TIMING
     if (tid == 0 && P.dbg_time) {
         tacc[8] = clock64() - tprev;
