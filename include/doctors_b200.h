@@ -114,8 +114,9 @@ typedef struct {
     int check_window;         /* tolerance mode: sweeps enqueued between host reads of the device flag; 0 = adaptive
                                * (first read one sweep before the count the previous group needed, then every sweep) */
     int projection;           /* sweep_mode 0, the two projections of Eq. (2) rhs / Eq. (3) inside the sweep kernel:
-                               * 0 automatic = tensor cores (mma TF32, 3-product split, fp32 accumulate) when P3 and the
-                               * octant has <= 48 directions, else packed fp32 FMA loops; 1 = always the fp32 FMA loops */
+                               * 0 automatic (= 1: the fastest measured on B200), 1 packed fp32 FMA loops,
+                               * 2 tensor cores (mma TF32, 3-product split, fp32 accumulate) when P3, <= 48 directions per
+                               *   octant and a brick of a multiple of 8 cells; else the FMA loops */
 } doctors_solve_opts;
 
 typedef struct {

@@ -33,7 +33,7 @@ struct GroupResult { int iters; int hit_max; float resid; float pad; double leak
 // Workspace layout for one choice of options.
 struct Plan {
     bool ok = false;
-    long long cells_p = 0; int NCb = 0;
+    long long cells_p = 0; int NCb = 0; int tm_inner = 0, tm_rows = 0;   // TMA box = tm_rows rows of tm_inner cells = one brick
     int MT = 0;                     // m-tiles of the tensor-core projections (0: FFMA2 loops), see sweep_brick.cuh
     int nprob = 0, chunk = 0, nchunks = 0, nsrc = 0, nvol = 0;
     int G = 0, L = 0, NM = 0, ndir = 0, M = 0;
@@ -104,7 +104,7 @@ int fail(doctors_problem* p, int code, const char* fmt, ...)
 
 int nprob_of(const doctors_problem* p) { return p->mode == 0 ? int(p->sources.size()) : 1; }
 
-void auto_brick(int NM, int M, int nx, int ny, int nz, const int* req, int B[3])
+void auto_brick(int NM, int M, int nx, int ny, int nz, const int* req, bool mt, int B[3])
 {
     if (req && req[0] > 0 && req[1] > 0 && req[2] > 0) { B[0] = req[0]; B[1] = req[1]; B[2] = req[2]; return; }
     // cross section = the 32 lanes of a warp (8 x 4, reshaped for thin meshes); BX as long as shared memory allows
@@ -114,7 +114,7 @@ void auto_brick(int NM, int M, int nx, int ny, int nz, const int* req, int B[3])
     const int cand[5] = {20, 16, 12, 8, 4};        // 20 x 8 x 4 = 640 cells = 2 per thread of a 320-thread CTA, 3 CTAs per SM
     for (int c = 0; c < 5; ++c) {
         B[0] = std::min(cand[c], (nx + 3) / 4 * 4);
-        if (brick_smem_layout(NM, B[0], B[1], B[2], M, projection_mtiles(NM, M, B[0] * B[1] * B[2])).total <= 74 * 1024) break;
+        if (brick_smem_layout(NM, B[0], B[1], B[2], M, mt ? projection_mtiles(NM, M, B[0] * B[1] * B[2]) : 0).total <= 74 * 1024) break;
     }
 }
 
@@ -132,16 +132,19 @@ Plan make_plan(const doctors_problem* p, const doctors_solve_opts* o, int chunk)
     P.sweep_mode = o ? o->sweep_mode : 0;
     P.deterministic = o ? o->deterministic : 0;
     for (auto& s : p->sources) if (s.kind == 0) ++P.nvol;
-    auto_brick(P.NM, P.M, p->nx, p->ny, p->nz, o ? o->brick : nullptr, P.B);
+    auto_brick(P.NM, P.M, p->nx, p->ny, p->nz, o ? o->brick : nullptr, o && o->projection == 2, P.B);
     P.gb[0] = (p->nx + P.B[0] - 1) / P.B[0];
     P.gb[1] = (p->ny + P.B[1] - 1) / P.B[1];
     P.gb[2] = (p->nz + P.B[2] - 1) / P.B[2];
     P.nbricks = (long long)P.gb[0] * P.gb[1] * P.gb[2];
     P.NCb = P.B[0] * P.B[1] * P.B[2];
     P.cells_p = P.nbricks * P.NCb;                              // brick-major storage, edge bricks padded
-    // one brick = NCb contiguous cells per moment: moved by 1-D bulk copies (16-byte multiples: BX % 4 == 0)
+    // one brick = NCb contiguous cells per moment; a TMA box row holds at most 256 elements and must be a 16-byte multiple
+    P.tm_rows = 1;
+    while ((P.NCb / 4) % P.tm_rows != 0 || P.NCb / P.tm_rows > 256) ++P.tm_rows;
+    P.tm_inner = P.NCb / P.tm_rows;
     P.ntasks = P.nbricks * 8 * P.chunk;
-    P.MT = (o && o->projection == 1) ? 0 : projection_mtiles(P.NM, P.M, P.NCb);
+    P.MT = (o && o->projection == 2) ? projection_mtiles(P.NM, P.M, P.NCb) : 0;
     P.smem = brick_smem_layout(P.NM, P.B[0], P.B[1], P.B[2], P.M, P.MT).total;
     { int dpw = (P.M + kMaxSweepWarps - 1) / kMaxSweepWarps; P.W = (P.M + dpw - 1) / dpw; }
 
@@ -456,7 +459,7 @@ int doctors_debug_schedule_dims(doctors_problem* p, const doctors_solve_opts* op
     if (level == 0) { dims[0] = p->nx; dims[1] = p->ny; dims[2] = p->nz; return DOCTORS_OK; }
     if (!p->has_xs || !p->has_quad) return fail(p, DOCTORS_BAD_STATE, "xs / quadrature not set (brick size depends on them)");
     int B[3];
-    auto_brick((p->L + 1) * (p->L + 1), p->ndir / 8, p->nx, p->ny, p->nz, opts ? opts->brick : nullptr, B);
+    auto_brick((p->L + 1) * (p->L + 1), p->ndir / 8, p->nx, p->ny, p->nz, opts ? opts->brick : nullptr, opts && opts->projection == 2, B);
     if (level == 1) { for (int a = 0; a < 3; ++a) dims[a] = ((a == 0 ? p->nx : a == 1 ? p->ny : p->nz) + B[a] - 1) / B[a]; return DOCTORS_OK; }
     if (level == 2) { for (int a = 0; a < 3; ++a) dims[a] = B[a]; return DOCTORS_OK; }
     return fail(p, DOCTORS_INVALID_ARG, "level must be 0, 1 or 2");
@@ -576,6 +579,7 @@ int make_tensor_map(doctors_problem* p, CUtensorMap* tm, void* base, int rank, c
 }
 
 struct SweepLaunch {
+    CUtensorMap tmQ, tmPhi;
     BrickParams bp;
     int grid = 0;
     size_t smem = 0;
@@ -584,7 +588,7 @@ struct SweepLaunch {
 template <int NM, bool FIX, int MT>
 cudaError_t launch_brick(const SweepLaunch& S, cudaStream_t st)
 {
-    k_sweep_brick<NM, FIX, MT><<<S.grid, 32 * S.bp.W, S.smem, st>>>(S.bp);
+    k_sweep_brick<NM, FIX, MT><<<S.grid, 32 * S.bp.W, S.smem, st>>>(S.tmQ, S.tmPhi, S.bp);
     return cudaGetLastError();
 }
 
@@ -820,6 +824,17 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         CK(cudaMemsetAsync(at<unsigned>(p, P.o_flags), 0, size_t(P.chunk) * 8 * P.nbricks * 4, st));
 
         {
+            // brick-major arrays: a brick's cells of one moment are tm_rows contiguous rows of tm_inner cells
+            cuuint64_t d4[4] = {cuuint64_t(P.tm_inner), cuuint64_t(P.tm_rows) * P.nbricks, cuuint64_t(NM), cuuint64_t(P.chunk)};
+            cuuint64_t s4[3] = {cuuint64_t(P.tm_inner) * 4, cuuint64_t(cp) * 4, cuuint64_t(cp) * NM * 4};
+            cuuint32_t b4[4] = {cuuint32_t(P.tm_inner), cuuint32_t(P.tm_rows), cuuint32_t(NM), 1};
+            rc = make_tensor_map(p, &SL.tmQ, at<float>(p, P.o_Q), 4, d4, s4, b4);
+            if (rc != DOCTORS_OK) return rc;
+            d4[3] = cuuint64_t(P.chunk) * G;
+            rc = make_tensor_map(p, &SL.tmPhi, at<float>(p, P.o_phiall), 4, d4, s4, b4);
+            if (rc != DOCTORS_OK) return rc;
+        }
+        {
             const std::vector<unsigned char> blob = build_octtabs(NM, M, P.MT, dird, lkc, Mt_f, Dt_f);
             CK(cudaMemcpyAsync(at<unsigned char>(p, P.o_octtab), blob.data(), blob.size(), cudaMemcpyHostToDevice, st));
             CK(cudaStreamSynchronize(st));
@@ -837,7 +852,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         bp.BX = P.B[0]; bp.BY = P.B[1]; bp.BZ = P.B[2];
         bp.gbx = P.gb[0]; bp.gby = P.gb[1]; bp.gbz = P.gb[2];
         bp.M = M; bp.W = P.W; bp.g = 0; bp.Gs = G; bp.epoch = 0;
-        bp.NCb = P.NCb; bp.cells_p = P.cells_p;
+        bp.NCb = P.NCb; bp.cells_p = P.cells_p; bp.tm_rows = P.tm_rows;
         bp.Q = at<float>(p, P.o_Q); bp.phi = at<float>(p, P.o_phiall); bp.sigt = at<double>(p, P.o_sigt);
         bp.octtab = at<unsigned char>(p, P.o_octtab);
         bp.tasks = at<uint2>(p, P.o_tasks);
@@ -1104,8 +1119,20 @@ extern "C" int doctors_debug_device_brick_steps(doctors_problem* p, int bx, int 
     }
     cudaMemcpy(S.task, &task, sizeof task, cudaMemcpyHostToDevice);
     SweepLaunch SL;
+    int rows = 1;
+    while ((NC / 4) % rows != 0 || NC / rows > 256) ++rows;
+    {
+        const int inner = NC / rows;
+        cuuint64_t d4[4] = {cuuint64_t(inner), cuuint64_t(rows), 1, 1};
+        cuuint64_t s4[3] = {cuuint64_t(inner) * 4, cuuint64_t(NC) * 4, cuuint64_t(NC) * 4};
+        cuuint32_t b4[4] = {cuuint32_t(inner), cuuint32_t(rows), 1, 1};
+        int rc = make_tensor_map(p, &SL.tmQ, S.Q, 4, d4, s4, b4);
+        if (rc == DOCTORS_OK) rc = make_tensor_map(p, &SL.tmPhi, S.phi, 4, d4, s4, b4);
+        if (rc != DOCTORS_OK) { cudaFree(base); return rc; }
+    }
     BrickParams& bp = SL.bp;
     std::memset(&bp, 0, sizeof bp);
+    bp.tm_rows = rows;
     bp.nx = bx; bp.ny = by; bp.nz = bz; bp.BX = bx; bp.BY = by; bp.BZ = bz; bp.gbx = bp.gby = bp.gbz = 1;
     bp.M = 1; bp.W = 1; bp.g = 0; bp.Gs = 1; bp.epoch = 1; bp.task_begin = 0; bp.ntasks = 1; bp.counter_slot = 0;
     bp.NCb = NC; bp.cells_p = NC; bp.Q = S.Q; bp.phi = S.phi; bp.sigt = S.sig; bp.octtab = S.tab;
@@ -1115,7 +1142,7 @@ extern "C" int doctors_debug_device_brick_steps(doctors_problem* p, int bx, int 
     bp.dbg_time = nullptr; bp.dbg_plane = S.planes;
     cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<1, false, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
     if (e == cudaSuccess) {
-        k_sweep_brick<1, false, 0, true><<<1, 32, smem, p->stream>>>(bp);
+        k_sweep_brick<1, false, 0, true><<<1, 32, smem, p->stream>>>(SL.tmQ, SL.tmPhi, bp);
         e = cudaGetLastError();
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);

@@ -41,6 +41,7 @@ struct BrickParams {
     int gbx, gby, gbz;           // brick grid
     int M;                       // directions per octant
     int NCb;                     // cells per brick (= BX*BY*BZ): brick b of a per-cell array starts at b * NCb
+    int tm_rows;                 // tensor maps of Q / phi: a brick = tm_rows box rows (coordinate 1 of brick b = tm_rows * b)
     long long cells_p;           // padded cell count (plane pitch of Q / phi in global memory)
     const float* Q;              // [prob][NM][cells_p]
     float* phi;                  // [prob * Gs + g][NM][cells_p]
@@ -285,7 +286,7 @@ __device__ __noinline__ void project_directions_to_moments_mma(uint32_t tile, ui
 
 template <int NM, bool FIX, int MT, bool DBG = false>
 __global__ void __launch_bounds__(32 * kMaxSweepWarps, 3)
-k_sweep_brick(const BrickParams P)
+k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmPhi, const BrickParams P)
 {
     static_assert(MT == 0 || NM == 16, "tensor-core projections are written for P3 (16 moments)");
     static_assert(NM <= 16, "one tile-warp lane per moment plane, lanes 16 / 17 for sigma_t and the tables");
@@ -402,7 +403,15 @@ k_sweep_brick(const BrickParams P)
             const bool tab = oct != last_oct;
             if (lane == 0) mbar_expect_tx(bar, uint32_t(NM * NC * 4 + NC * 8 + (tab ? T.total : 0)));
             const float* gq = P.Q + (size_t)prob * NM * P.cells_p + (size_t)brick * P.NCb;
-            if (lane < NM) {
+            if constexpr (MT == 0) {
+                // dense tile [NM][brick]: ONE tensor copy (4-D box {row, rows of the brick, moments, problem}); issuing a bulk
+                // operation costs ~200 cycles of the issuing warp, so one per moment plane is only used where the planes
+                // are padded in shared memory (tensor-core projections)
+                if (lane == 0) {
+                    bulk_wait_read0();                           // the reduce-add of the previous task has read the tile
+                    tma_load_4d(smem_u32(sQ), &tmQ, bar, 0, P.tm_rows * brick, 0, prob);
+                }
+            } else if (lane < NM) {
                 bulk_wait_read0();                               // this lane's reduce-add of the previous task has read its plane
                 bulk_load(smem_u32(sQ + lane * NCP), gq + (size_t)lane * P.cells_p, uint32_t(NC * 4), bar);
             }
@@ -650,10 +659,17 @@ k_sweep_brick(const BrickParams P)
         fence_proxy_async_smem();
         __syncthreads();
         TICK(7);
-        if (warp == tileWarp && lane < NM) {
-            float* gphi = P.phi + (size_t)(prob * P.Gs + P.g) * NM * P.cells_p + (size_t)brick * P.NCb;
-            bulk_reduce_add_f32(gphi + (size_t)lane * P.cells_p, smem_u32(sQ + lane * NCP), uint32_t(NC * 4));
-            bulk_commit();
+        if (warp == tileWarp) {
+            if constexpr (MT == 0) {
+                if (lane == 0) {
+                    tma_reduce_add_4d(&tmPhi, smem_u32(sQ), 0, P.tm_rows * brick, 0, prob * P.Gs + P.g);
+                    bulk_commit();
+                }
+            } else if (lane < NM) {
+                float* gphi = P.phi + (size_t)(prob * P.Gs + P.g) * NM * P.cells_p + (size_t)brick * P.NCb;
+                bulk_reduce_add_f32(gphi + (size_t)lane * P.cells_p, smem_u32(sQ + lane * NCP), uint32_t(NC * 4));
+                bulk_commit();
+            }
         }
         if (tid == 0 && (edge_x | edge_y | edge_z)) {
             float s = 0.0f;
