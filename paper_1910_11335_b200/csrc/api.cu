@@ -852,7 +852,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         bp.BX = P.B[0]; bp.BY = P.B[1]; bp.BZ = P.B[2];
         bp.gbx = P.gb[0]; bp.gby = P.gb[1]; bp.gbz = P.gb[2];
         bp.M = M; bp.W = P.W; bp.g = 0; bp.Gs = G; bp.epoch = 0;
-        bp.NCb = P.NCb; bp.cells_p = P.cells_p; bp.tm_rows = P.tm_rows;
+        bp.NCb = P.NCb; bp.cells_p = P.cells_p; bp.tm_rows = P.tm_rows; bp.nprob = P.chunk;
         bp.Q = at<float>(p, P.o_Q); bp.phi = at<float>(p, P.o_phiall); bp.sigt = at<double>(p, P.o_sigt);
         bp.octtab = at<unsigned char>(p, P.o_octtab);
         bp.tasks = at<uint2>(p, P.o_tasks);
@@ -1132,7 +1132,7 @@ extern "C" int doctors_debug_device_brick_steps(doctors_problem* p, int bx, int 
     }
     BrickParams& bp = SL.bp;
     std::memset(&bp, 0, sizeof bp);
-    bp.tm_rows = rows;
+    bp.tm_rows = rows; bp.nprob = 1;
     bp.nx = bx; bp.ny = by; bp.nz = bz; bp.BX = bx; bp.BY = by; bp.BZ = bz; bp.gbx = bp.gby = bp.gbz = 1;
     bp.M = 1; bp.W = 1; bp.g = 0; bp.Gs = 1; bp.epoch = 1; bp.task_begin = 0; bp.ntasks = 1; bp.counter_slot = 0;
     bp.NCb = NC; bp.cells_p = NC; bp.Q = S.Q; bp.phi = S.phi; bp.sigt = S.sig; bp.octtab = S.tab;

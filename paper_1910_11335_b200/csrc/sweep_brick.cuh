@@ -40,6 +40,7 @@ struct BrickParams {
     int BX, BY, BZ;              // brick extents (BX % 4 == 0, BY * BZ <= 32)
     int gbx, gby, gbz;           // brick grid
     int M;                       // directions per octant
+    int nprob;                   // problems the task list refers to (<= 256)
     int NCb;                     // cells per brick (= BX*BY*BZ): brick b of a per-cell array starts at b * NCb
     int tm_rows;                 // tensor maps of Q / phi: a brick = tm_rows box rows (coordinate 1 of brick b = tm_rows * b)
     long long cells_p;           // padded cell count (plane pitch of Q / phi in global memory)
@@ -98,7 +99,7 @@ __host__ __device__ inline int plane_pitch(int NC, int MT)
 }
 
 struct BrickSmem {
-    size_t q, sig, psi, fx, fy, fz, tab, misc, total;
+    size_t q, sig, psi, fx, fy, fz, tab, done, misc, total;
 };
 
 __host__ __device__ inline BrickSmem brick_smem_layout(int NM, int BX, int BY, int BZ, int M, int MT)
@@ -115,6 +116,7 @@ __host__ __device__ inline BrickSmem brick_smem_layout(int NM, int BX, int BY, i
     s.fy = o;    o = align_up(o + size_t(M) * BX * BZ * 8, 8);
     s.fz = o;    o = align_up(o + size_t(M) * BX * BY * 8, 16);
     s.tab = o;   o = align_up(o + octtab_layout(NM, M, MT).total, 16);
+    s.done = o;  o = align_up(o + 256, 16);      // "problem has stopped" bytes of the launch (task prob index is 8 bits)
     o = align_up(o + 128, 16);                  // tail pad (idle lanes may read up to 10 cells past the tables' start)
     s.total = o;
     return s;
@@ -335,8 +337,8 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
     //   tile warp   lanes 0..NM-1 own one moment plane each: bulk load of Q_lm at the start of a task, bulk reduce-add of
     //               the phi_lm contribution at its end (same lane = same bulk group, so the lane can wait for "read done")
     //   pollers     warp 0, lanes 0..2: wait for the upwind brick in x / y / z and issue that face's bulk load themselves
-    //   prefetcher  one thread fetches the NEXT task (id from the atomic counter, descriptor, done flag of its problem)
-    //               into shared memory while the current one runs: three dependent global round trips off the critical path.
+    //   prefetcher  one thread fetches the NEXT task (id from the atomic counter, then its descriptor) into shared memory
+    //               while the current one runs: two dependent global round trips off the critical path.
     //               Holding one unstarted task cannot deadlock: a CTA's held task has a higher index than its running one,
     //               so the lowest unfinished task of the whole grid is always running.
     //   publisher   last lane of the last warp: bulk-stores the outflow faces, and at the next loop top waits for them and
@@ -346,13 +348,13 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
     const int pfThread = nwarps > 2 ? 64 : 32 * tileWarp + 8;
     const int pubWarp = nwarps - 1;
     uint2* sDesc = reinterpret_cast<uint2*>(smem + L.misc + 16);   // [2]
-    int* sDone = reinterpret_cast<int*>(smem + L.misc + 104);      // [2]
+    unsigned char* sDoneP = smem + L.done;                        // [nprob]: fixed for the whole launch (k_check runs between launches)
+    for (int q = tid; q < P.nprob; q += nthr) sDoneP[q] = (unsigned char)(__ldcg(&P.state[q].done) != 0);
     auto fetch_task = [&](int sl) {
         const int id = int(atomicAdd(&P.ctl->counters[P.counter_slot], 1u));
         uint2 d = make_uint2(0u, 0u);
-        int dn = 0;
-        if (id < P.ntasks) { d = P.tasks[P.task_begin + id]; dn = __ldcg(&P.state[d.x & 0xff].done); }
-        sDesc[sl] = d; sDone[sl] = dn; sTask[sl] = id;
+        if (id < P.ntasks) d = P.tasks[P.task_begin + id];
+        sDesc[sl] = d; sTask[sl] = id;
     };
     if (tid == 0) fetch_task(0);
     int slot = 0;
@@ -373,7 +375,7 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         const int t = sTask[slot];
         if (t >= P.ntasks) break;
         const uint2 td = sDesc[slot];
-        const int prob_done = sDone[slot];
+        const int prob_done = sDoneP[td.x & 0xff];
         if (tid == pfThread) fetch_task(slot ^ 1);
         slot ^= 1;
         TICK(0);
