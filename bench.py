@@ -44,6 +44,20 @@ def measured_peak():
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def ncu_traffic_per_problem_sweep(idx):
+    """DRAM bytes (read + write) one problem's share of a sweep launch moved under `ncu --set full`, from the committed
+    summary profiles/r01_sweep_traffic.csv (columns: config, problems_in_launch, dram_read_bytes, dram_write_bytes)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r01_sweep_traffic.csv")) as f:
+            for ln in f:
+                c = ln.strip().split(",")
+                if len(c) >= 4 and c[0].strip() == str(idx):
+                    return (float(c[2]) + float(c[3])) / float(c[1])
+    except Exception:
+        pass
+    return None
+
+
 def workload_for(idx, slice_=False):
     from workloads import make_config, single_sweep_case
     if slice_:
@@ -296,8 +310,13 @@ def run_gpu_arm(args):
     problem_sweeps = updates / (wl.cells * wl.n_dir)               # sum of K[s][g] over the timed steps
     alg_bytes = problem_sweeps * wl.cells * 8 * bytes_per
     achieved = alg_bytes / (ms_sweep * 1e-3) / 1e9
+    traffic = args.traffic
+    if traffic is None:
+        per = ncu_traffic_per_problem_sweep(args.config)          # one ncu capture, scaled to this run's problems per launch
+        if per is not None:
+            traffic = per * problem_sweeps / max(1, sweep_launches)
     roofline = {"bound": "hbm", "kernel": "k_sweep_brick", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "peak_source": peak_src, "traffic": args.traffic,
+                "frac": achieved / peak, "peak_source": peak_src, "traffic": traffic, "traffic_unit": "DRAM bytes per launch (ncu, profiles/r01_sweep_traffic.csv)",
                 "launches": int(sweep_launches), "avg_launch_ms": ms_sweep / max(1, sweep_launches),
                 "algorithmic_bytes_per_launch": alg_bytes / max(1, sweep_launches),
                 "share_of_step": ms_sweep / ms_dev,
