@@ -52,7 +52,7 @@ class CSolveInfo(C.Structure):
                 ("ms_iterate", C.c_double), ("ms_total", C.c_double),
                 ("updates", C.c_ulonglong), ("sweep_launches", C.c_ulonglong), ("kernel_launches", C.c_ulonglong),
                 ("n_chunks", C.c_int), ("brick", C.c_int * 3), ("ctas_per_sm", C.c_int),
-                ("projection_mtiles", C.c_int)]
+                ("sweep_kernel", C.c_int), ("projection_mtiles", C.c_int)]
 
 
 _lib = None
@@ -288,7 +288,7 @@ class Problem:
                     ms_iterate=info.ms_iterate, ms_total=info.ms_total, updates=int(info.updates),
                     sweep_launches=int(info.sweep_launches), kernel_launches=int(info.kernel_launches),
                     n_chunks=info.n_chunks, brick=tuple(info.brick), ctas_per_sm=info.ctas_per_sm,
-                    projection_mtiles=info.projection_mtiles)
+                    projection_mtiles=info.projection_mtiles, sweep_kernel=info.sweep_kernel)
 
     # ---- get_* ------------------------------------------------------------------------------
     def get_flux_moments(self, problem, group, l_max=0, out=None):

@@ -16,6 +16,7 @@
 #include "host_tables.h"
 #include "kernels.cuh"
 #include "sweep_brick.cuh"
+#include "sweep_row.cuh"
 
 using namespace doctors;
 
@@ -38,6 +39,8 @@ struct Plan {
     int nprob = 0, chunk = 0, nchunks = 0, nsrc = 0, nvol = 0;
     int G = 0, L = 0, NM = 0, ndir = 0, M = 0;
     int mode = 0, sweep_mode = 0, deterministic = 0;
+    bool row = false;               // sweep_mode 2 accepted: the row-pipelined kernel (same workspace and set-up as mode 0)
+    size_t row_smem = 0;
     int B[3] = {0, 0, 0}, gb[3] = {0, 0, 0};
     int W = 1;                      // sweep warps per CTA
     long long nbricks = 0, ntasks = 0;
@@ -145,6 +148,15 @@ Plan make_plan(const doctors_problem* p, const doctors_solve_opts* o, int chunk)
     P.tm_inner = P.NCb / P.tm_rows;
     P.ntasks = P.nbricks * 8 * P.chunk;
     P.MT = (o && o->projection == 2) ? projection_mtiles(P.NM, P.M, P.NCb) : 0;
+    if (P.sweep_mode == 2) {
+        // row-pipelined kernel where it applies (sweep_row.cuh), else the brick kernel; everything around the launch is mode 0
+        const int skew = P.B[1] + P.B[2] - 2, rest = p->nx % P.B[0];
+        P.row_smem = row_smem_layout(P.NM, P.B[0], P.B[1], P.B[2], P.M).total;
+        P.row = P.M <= kMaxSweepWarps && (size_t(P.M) * P.B[0] * P.B[2]) % 2 == 0 && (size_t(P.M) * P.B[0] * P.B[1]) % 2 == 0 &&
+                P.B[0] >= skew && (rest == 0 || rest >= skew) && P.row_smem <= 227 * 1024 && P.chunk <= 255;
+        P.sweep_mode = 0;
+        if (P.row) P.MT = 0;
+    }
     P.smem = brick_smem_layout(P.NM, P.B[0], P.B[1], P.B[2], P.M, P.MT).total;
     { int dpw = (P.M + kMaxSweepWarps - 1) / kMaxSweepWarps; P.W = (P.M + dpw - 1) / dpw; }
 
@@ -593,6 +605,19 @@ cudaError_t launch_brick(const SweepLaunch& S, cudaStream_t st)
 }
 
 template <int NM, bool FIX, int MT>
+cudaError_t launch_row(const SweepLaunch& S, const RowParams& rp, int grid, size_t smem, cudaStream_t st)
+{
+    k_sweep_row<NM, FIX><<<grid, kRowThreads, smem, st>>>(S.tmQ, S.tmPhi, rp);
+    return cudaGetLastError();
+}
+
+template <int NM, bool FIX, int MT>
+cudaError_t prep_row(size_t smem)
+{
+    return cudaFuncSetAttribute(k_sweep_row<NM, FIX>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+}
+
+template <int NM, bool FIX, int MT>
 cudaError_t prep_brick(size_t smem, int threads, int* max_ctas)
 {
     cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<NM, FIX, MT>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
@@ -694,7 +719,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
     const bool adaptive_window = o.check_window <= 0;   // first host read where the previous group stopped, then every sweep
     if (o.check_window <= 0) o.check_window = 12;
     if (o.closure != 0 && o.closure != 1) return fail(p, DOCTORS_INVALID_ARG, "closure must be 0 or 1");
-    if (o.sweep_mode != 0 && o.sweep_mode != 1) return fail(p, DOCTORS_INVALID_ARG, "sweep_mode must be 0 or 1");
+    if (o.sweep_mode < 0 || o.sweep_mode > 2) return fail(p, DOCTORS_INVALID_ARG, "sweep_mode must be 0, 1 or 2");
     if (o.brick[0] > 0 && (o.brick[0] % 4 != 0 || o.brick[0] > 64 || o.brick[1] <= 0 || o.brick[2] <= 0 || o.brick[1] * o.brick[2] > 32))
         return fail(p, DOCTORS_INVALID_ARG, "brick: brick[0] a multiple of 4 (<= 64), brick[1] * brick[2] <= 32 (the lanes of a warp)");
     if (!p->ws) return fail(p, DOCTORS_ALLOC, "no workspace set");
@@ -792,6 +817,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
     std::vector<int> oct_begin(9, 0);
     std::vector<std::vector<int32_t>> sched_off(8);
     SweepLaunch SL;
+    RowParams rowp;
     int ctas_per_sm = 0;
     if (P.sweep_mode == 0) {
         // level 2 (cells of a brick) needs no table: lane (j',k') at step s updates i' = s - j' - k' (Eq. 8)
@@ -804,7 +830,30 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
             int bi = b % P.gb[0], bj = (b / P.gb[0]) % P.gb[1], bk = b / (P.gb[0] * P.gb[1]);
             tasks.push_back(make_uint2(uint32_t(q) | uint32_t(oc) << 8, uint32_t(bi) | uint32_t(bj) << 10 | uint32_t(bk) << 20));
         };
-        if (!P.deterministic) {
+        if (P.row) {
+            // row tasks (problem, octant, bj, bk) in sub-sweep order of the (bj, bk) grid (Eq. 8 in two dimensions)
+            std::vector<std::vector<int32_t>> roff(8), rcell(8);
+            for (int oc = 0; oc < 8; ++oc) subsweep_schedule(1, P.gb[1], P.gb[2], oc, roff[oc], rcell[oc]);
+            const int rplanes = P.gb[1] + P.gb[2] - 1;
+            auto pushr = [&](int q, int oc, int r) {
+                tasks.push_back(make_uint2(uint32_t(q) | uint32_t(oc) << 8, uint32_t(r % P.gb[1]) | uint32_t(r / P.gb[1]) << 10));
+            };
+            if (!P.deterministic) {
+                for (int S = 0; S < rplanes; ++S)
+                    for (int q = 0; q < P.chunk; ++q)
+                        for (int oc = 0; oc < 8; ++oc)
+                            for (int t = roff[oc][S]; t < roff[oc][S + 1]; ++t) pushr(q, oc, rcell[oc][t]);
+                oct_begin[0] = 0; oct_begin[1] = int(tasks.size());
+            } else {
+                for (int oc = 0; oc < 8; ++oc) {
+                    oct_begin[oc] = int(tasks.size());
+                    for (int S = 0; S < rplanes; ++S)
+                        for (int q = 0; q < P.chunk; ++q)
+                            for (int t = roff[oc][S]; t < roff[oc][S + 1]; ++t) pushr(q, oc, rcell[oc][t]);
+                }
+                oct_begin[8] = int(tasks.size());
+            }
+        } else if (!P.deterministic) {
             // all problems and octants interleaved, brick sub-sweep S outermost
             for (int S = 0; S < gplanes; ++S)
                 for (int q = 0; q < P.chunk; ++q)
@@ -847,6 +896,22 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         ctas_per_sm = o.ctas_per_sm > 0 ? std::min(o.ctas_per_sm, max_ctas) : max_ctas;
         SL.grid = p->num_sms * ctas_per_sm;
         SL.smem = P.smem;
+        if (P.row) {
+            DISPATCH_NM_FIX(NM, o.closure == 1, 0, e = (prep_row<NM, FIX, MT>(P.row_smem)));
+            if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "row sweep kernel setup failed: %s (smem %zu)", cudaGetErrorString(e), P.row_smem);
+            ctas_per_sm = 1;
+            RowParams& r = rowp;
+            std::memset(&r, 0, sizeof r);
+            r.nx = nx; r.ny = ny; r.nz = nz; r.BX = P.B[0]; r.BY = P.B[1]; r.BZ = P.B[2];
+            r.gbx = P.gb[0]; r.gby = P.gb[1]; r.gbz = P.gb[2]; r.M = M; r.nprob = P.chunk; r.NCb = P.NCb; r.cells_p = P.cells_p;
+            r.tm_rows = P.tm_rows; r.sigt = at<double>(p, P.o_sigt); r.octtab = at<unsigned char>(p, P.o_octtab);
+            r.Gs = G; r.tasks = at<uint2>(p, P.o_tasks); r.ctl = at<Control>(p, P.o_ctl); r.flags = at<unsigned>(p, P.o_flags);
+            r.faceY = at<double>(p, P.o_fy); r.faceZ = at<double>(p, P.o_fz);
+            r.state = at<ProbState>(p, P.o_state); r.leak = at<double>(p, P.o_leak);
+#ifdef DOCTORS_TIMING
+            { static long long* dt = nullptr; if (!dt) { cudaMalloc(&dt, 32 * 8); } cudaMemset(dt, 0, 32 * 8); r.dbg_time = dt; }
+#endif
+        }
         BrickParams& bp = SL.bp;
         bp.nx = nx; bp.ny = ny; bp.nz = nz;
         bp.BX = P.B[0]; bp.BY = P.B[1]; bp.BZ = P.B[2];
@@ -967,6 +1032,11 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
                             // problems done (k_group_begin), so their tasks are skipped
                             SL.bp.ntasks = oct_begin[l + 1] - oct_begin[l];
                             cudaError_t e;
+                            if (P.row) {
+                                rowp.g = g; rowp.epoch = SL.bp.epoch; rowp.counter_slot = l;
+                                rowp.task_begin = SL.bp.task_begin; rowp.ntasks = SL.bp.ntasks;
+                                DISPATCH_NM_FIX(NM, o.closure == 1, 0, e = (launch_row<NM, FIX, MT>(SL, rowp, p->num_sms, P.row_smem, st)));
+                            } else
                             DISPATCH_NM_FIX(NM, o.closure == 1, P.MT, e = (launch_brick<NM, FIX, MT>(SL, st)));
                             if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "sweep launch failed: %s", cudaGetErrorString(e));
                             ++sweep_launches; ++kernel_launches;
@@ -1017,7 +1087,15 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
     CK(cudaGetLastError());
 
 #ifdef DOCTORS_TIMING
-    if (P.sweep_mode == 0 && SL.bp.dbg_time) {
+    if (P.row && rowp.dbg_time) {
+        long long h[32];
+        cudaMemcpy(h, rowp.dbg_time, sizeof h, cudaMemcpyDeviceToHost);
+        const char* nm[20] = {"loader total", "loader wait phase 2", "loader wait reduce read", "-", "z poller total", "poller wait face slot", "poller flag spin", "-",
+                              "publisher total", "publisher wait wave", "publisher wait store", "-", "proj total", "proj wait tile", "proj wait wave", "-",
+                              "wave total", "wave wait phase 0", "wave wait faces", "-"};
+        for (int i = 0; i < 20; ++i) if (nm[i][0] != '-') fprintf(stderr, "  [row timing] %-26s %.3e cycles (%5.1f %% of its role)\n", nm[i], double(h[i]), 100.0 * h[i] / double(h[i / 4 * 4]));
+    }
+    if (!P.row && P.sweep_mode == 0 && SL.bp.dbg_time) {
         long long h[16];
         cudaMemcpy(h, SL.bp.dbg_time, sizeof h, cudaMemcpyDeviceToHost);
         const char* nm[12] = {"fetch", "dep: tables+sync", "face-load", "tma-wait", "phase0", "wavefront", "face-store+release", "phase2", "tail", "dep: reduce-read wait + TMA issue", "dep: flag poll", "-"};
@@ -1054,6 +1132,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         info->brick[0] = P.B[0]; info->brick[1] = P.B[1]; info->brick[2] = P.B[2];
         info->ctas_per_sm = ctas_per_sm;
         info->projection_mtiles = P.sweep_mode == 0 ? P.MT : 0;
+        info->sweep_kernel = o.sweep_mode == 1 ? 1 : (P.row ? 2 : 0);
     }
     for (auto e : sweep_ev) cudaEventDestroy(e);
     for (auto e : fixed_ev) cudaEventDestroy(e);
