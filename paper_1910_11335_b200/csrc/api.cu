@@ -40,6 +40,7 @@ struct Plan {
     int G = 0, L = 0, NM = 0, ndir = 0, M = 0;
     int mode = 0, sweep_mode = 0, deterministic = 0;
     bool row = false;               // sweep_mode 2 accepted: the row-pipelined kernel (same workspace and set-up as mode 0)
+    int row_cfg = 0;                // 0: one CTA per SM, 3 stages (A); 1: two CTAs per SM, 2 stages (B)
     size_t row_smem = 0;
     int B[3] = {0, 0, 0}, gb[3] = {0, 0, 0};
     int W = 1;                      // sweep warps per CTA
@@ -151,9 +152,14 @@ Plan make_plan(const doctors_problem* p, const doctors_solve_opts* o, int chunk)
     if (P.sweep_mode == 2) {
         // row-pipelined kernel where it applies (sweep_row.cuh), else the brick kernel; everything around the launch is mode 0
         const int skew = P.B[1] + P.B[2] - 2, rest = p->nx % P.B[0];
-        P.row_smem = row_smem_layout(P.NM, P.B[0], P.B[1], P.B[2], P.M).total;
-        P.row = P.M <= kMaxSweepWarps && (size_t(P.M) * P.B[0] * P.B[2]) % 2 == 0 && (size_t(P.M) * P.B[0] * P.B[1]) % 2 == 0 &&
-                P.B[0] >= skew && (rest == 0 || rest >= skew) && P.row_smem <= 227 * 1024 && P.chunk <= 255;
+        const bool shape_ok = P.M <= kMaxSweepWarps && (size_t(P.M) * P.B[0] * P.B[2]) % 2 == 0 && (size_t(P.M) * P.B[0] * P.B[1]) % 2 == 0 &&
+                              P.B[0] >= skew && (rest == 0 || rest >= skew) && P.chunk <= 255;
+        const size_t smemA = row_smem_layout(P.NM, P.B[0], P.B[1], P.B[2], P.M, 3).total;
+        const size_t smemB = row_smem_layout(P.NM, P.B[0], P.B[1], P.B[2], P.M, 2).total;
+        // A (one CTA per SM, 3 stages) where it fits, else B (two CTAs per SM, 2 stages); measured equal on config 4
+        const bool fitB = smemB <= 113 * 1024, fitA = smemA <= 227 * 1024;
+        if (shape_ok && fitA) { P.row = true; P.row_cfg = 0; P.row_smem = smemA; }
+        else if (shape_ok && fitB) { P.row = true; P.row_cfg = 1; P.row_smem = smemB; }
         P.sweep_mode = 0;
         if (P.row) P.MT = 0;
     }
@@ -605,16 +611,18 @@ cudaError_t launch_brick(const SweepLaunch& S, cudaStream_t st)
 }
 
 template <int NM, bool FIX, int MT>
-cudaError_t launch_row(const SweepLaunch& S, const RowParams& rp, int grid, size_t smem, cudaStream_t st)
+cudaError_t launch_row(const SweepLaunch& S, const RowParams& rp, int cfg, int num_sms, size_t smem, cudaStream_t st)
 {
-    k_sweep_row<NM, FIX><<<grid, kRowThreads, smem, st>>>(S.tmQ, S.tmPhi, rp);
+    if (cfg == 1) k_sweep_row<NM, FIX, 2, 4, 2, 2><<<2 * num_sms, row_threads<2, 4>(), smem, st>>>(S.tmQ, S.tmPhi, rp);
+    else k_sweep_row<NM, FIX, 3, 5, 4, 1><<<num_sms, row_threads<3, 5>(), smem, st>>>(S.tmQ, S.tmPhi, rp);
     return cudaGetLastError();
 }
 
 template <int NM, bool FIX, int MT>
-cudaError_t prep_row(size_t smem)
+cudaError_t prep_row(int cfg, size_t smem)
 {
-    return cudaFuncSetAttribute(k_sweep_row<NM, FIX>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+    if (cfg == 1) return cudaFuncSetAttribute(k_sweep_row<NM, FIX, 2, 4, 2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+    return cudaFuncSetAttribute(k_sweep_row<NM, FIX, 3, 5, 4, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
 }
 
 template <int NM, bool FIX, int MT>
@@ -897,9 +905,9 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         SL.grid = p->num_sms * ctas_per_sm;
         SL.smem = P.smem;
         if (P.row) {
-            DISPATCH_NM_FIX(NM, o.closure == 1, 0, e = (prep_row<NM, FIX, MT>(P.row_smem)));
+            DISPATCH_NM_FIX(NM, o.closure == 1, 0, e = (prep_row<NM, FIX, MT>(P.row_cfg, P.row_smem)));
             if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "row sweep kernel setup failed: %s (smem %zu)", cudaGetErrorString(e), P.row_smem);
-            ctas_per_sm = 1;
+            ctas_per_sm = P.row_cfg == 1 ? 2 : 1;
             RowParams& r = rowp;
             std::memset(&r, 0, sizeof r);
             r.nx = nx; r.ny = ny; r.nz = nz; r.BX = P.B[0]; r.BY = P.B[1]; r.BZ = P.B[2];
@@ -1035,7 +1043,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
                             if (P.row) {
                                 rowp.g = g; rowp.epoch = SL.bp.epoch; rowp.counter_slot = l;
                                 rowp.task_begin = SL.bp.task_begin; rowp.ntasks = SL.bp.ntasks;
-                                DISPATCH_NM_FIX(NM, o.closure == 1, 0, e = (launch_row<NM, FIX, MT>(SL, rowp, p->num_sms, P.row_smem, st)));
+                                DISPATCH_NM_FIX(NM, o.closure == 1, 0, e = (launch_row<NM, FIX, MT>(SL, rowp, P.row_cfg, p->num_sms, P.row_smem, st)));
                             } else
                             DISPATCH_NM_FIX(NM, o.closure == 1, P.MT, e = (launch_brick<NM, FIX, MT>(SL, st)));
                             if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "sweep launch failed: %s", cudaGetErrorString(e));

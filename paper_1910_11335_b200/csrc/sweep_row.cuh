@@ -21,11 +21,14 @@
 
 namespace doctors {
 
-constexpr int kRowStages = 3;         // tile / face buffers in flight
 constexpr int kRowRing = 8;           // brick descriptors of the stream kept in shared memory
-constexpr int kRowProjWarps = 5;      // projection warps: 4 cells per thread on a 640-cell brick
-constexpr int kRowCtlWarps = 4;       // loader, y poller, z poller, publisher
-constexpr int kRowThreads = 32 * (kMaxSweepWarps + kRowProjWarps + kRowCtlWarps);
+constexpr int kRowTabRing = 4;        // octant table blobs kept in shared memory (a row names its slot)
+// Two configurations (template parameters of the kernel):
+//   A  one CTA per SM, 3 stages, 5 projection warps with 4 cells per thread (96 registers): no stage ever waited for
+//   B  two CTAs per SM, 2 stages, 4 projection warps with 2 cells per thread (64 registers): twice the wavefront warps per
+//      SM; a stage is recycled (phase 2 -> reduce-add -> next load -> phase 0) while the wavefront is on the other one
+// The control warp's lanes 0..3 are the loader, the y poller, the z poller and the publisher.
+template <int STAGES, int PW> constexpr int row_threads() { return 32 * (kMaxSweepWarps + PW + 1); }
 
 struct RowParams {
     int nx, ny, nz;
@@ -58,30 +61,32 @@ struct RowDesc {
     int bi, bj, bk;                  // brick
     int first, last;                 // first / last brick of its row
     int stop;                        // 1: end of the stream (no brick)
+    int tab;                         // slot of the octant's table blob in shared memory
+    int pad[3];
 };
 
 struct RowSmem {
     size_t bars, desc, lead, tile, sig, face, tab, done, total;
 };
-__host__ __device__ inline RowSmem row_smem_layout(int NM, int BX, int BY, int BZ, int M)
+__host__ __device__ inline RowSmem row_smem_layout(int NM, int BX, int BY, int BZ, int M, int stages)
 {
     RowSmem s;
     const size_t NC = size_t(BX) * BY * BZ;
     size_t o = 0;
-    s.bars = o;  o += 8 * 8 * kRowStages;                        // 8 mbarrier kinds x stages
+    s.bars = o;  o += 8 * 8 * size_t(stages);                    // 8 mbarrier kinds x stages
     s.desc = o;  o += sizeof(RowDesc) * kRowRing;
     s.lead = o;  o = align_up(o + 64, 128);
-    s.tile = o;  o = align_up(o + kRowStages * size_t(NM > M ? NM : M) * NC * 4, 128);
-    s.sig = o;   o = align_up(o + kRowStages * NC * 8, 128);
-    s.face = o;  o = align_up(o + kRowStages * size_t(M) * (size_t(BX) * BZ + size_t(BX) * BY) * 8, 128);
-    s.tab = o;   o = align_up(o + 8 * octtab_layout(NM, M, 0).total, 16);
+    s.tile = o;  o = align_up(o + stages * size_t(NM > M ? NM : M) * NC * 4, 128);
+    s.sig = o;   o = align_up(o + stages * NC * 8, 128);
+    s.face = o;  o = align_up(o + stages * size_t(M) * (size_t(BX) * BZ + size_t(BX) * BY) * 8, 128);
+    s.tab = o;   o = align_up(o + kRowTabRing * octtab_layout(NM, M, 0).total, 16);
     s.done = o;  o = align_up(o + 256, 16);
     o = align_up(o + 128, 16);                                   // tail pad (idle lanes read past the end of their arrays)
     s.total = o;
     return s;
 }
 
-// mbarrier kinds (index = kind * kRowStages + stage)
+// mbarrier kinds (index = kind * STAGES + stage)
 enum { kBarQ = 0,        // tile + sigma_t landed (tx bytes; armed by the loader)
        kBarPsi = 1,      // phase 0 done: q_n in place (projection warps arrive)
        kBarWave = 2,     // wavefront done on this tile: psi_n in place, outflow faces written (wavefront warps arrive)
@@ -108,16 +113,17 @@ __device__ __forceinline__ void sts_volatile_s32(uint32_t a, int v) { asm volati
 
 
 // ---- kernel ----------------------------------------------------------------------------------------------------
-template <int NM, bool FIX>
-__global__ void __launch_bounds__(kRowThreads, 1)
+template <int NM, bool FIX, int STAGES, int PW, int CPT, int CTAS>
+__global__ void __launch_bounds__((row_threads<STAGES, PW>()), CTAS)
 k_sweep_row(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmPhi, const RowParams P)
 {
     static_assert(NM <= 16, "moment planes");
+    constexpr int kRowStages = STAGES, kRowProjWarps = PW;
     if (__ldcg(&P.ctl->all_done)) return;
     extern __shared__ __align__(128) unsigned char smem[];
     const int BX = P.BX, BY = P.BY, BZ = P.BZ, M = P.M;
     const int NC = BX * BY * BZ;
-    const RowSmem L = row_smem_layout(NM, BX, BY, BZ, M);
+    const RowSmem L = row_smem_layout(NM, BX, BY, BZ, M, STAGES);
     const OctTab T = octtab_layout(NM, M, 0);
     const int planes = NM > M ? NM : M;
     const uint32_t sb = smem_u32(smem);
@@ -150,9 +156,7 @@ k_sweep_row(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
         fence_mbar_init();
         sts_volatile_s32(leadAddr, 0);
     }
-    // all 8 octants' tables and the stopped-problem bytes: once per launch
-    for (int e = tid; e < int(8 * T.total / 4); e += blockDim.x)
-        reinterpret_cast<uint32_t*>(smem + L.tab)[e] = __ldg(reinterpret_cast<const uint32_t*>(P.octtab) + e);
+    // the stopped-problem bytes: once per launch
     for (int q = tid; q < P.nprob; q += blockDim.x) sDoneP[q] = (unsigned char)(__ldcg(&P.state[q].done) != 0);
     __syncthreads();
 
@@ -173,12 +177,13 @@ k_sweep_row(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
         __threadfence_block();
         return sDesc[c % kRowRing];
     };
-    auto tab_of = [&](int oct) { return smem + L.tab + size_t(oct) * T.total; };
+    auto tab_of = [&](int slot) { return smem + L.tab + size_t(slot) * T.total; };
 
     // ================================================================================================================
     if (warp == ctlW0) {
-        // ---- loader (one lane): row tasks -> brick stream, tile loads two bricks ahead, reduce-adds behind phase 2 ----
+        // ---- loader (lane 0): row tasks -> brick stream, tile loads ahead of phase 0, reduce-adds behind phase 2 ----
         if (lane == 0) {
+            int tabslot = -1, taboct = -1;
             int c = 0;
             int next_id = int(atomicAdd(&P.ctl->counters[P.counter_slot], 1u));
             bool more = true;
@@ -193,11 +198,13 @@ k_sweep_row(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
                 }
                 const int nb = have ? P.gbx : 1;                 // the stop marker takes one stream position
                 const int oct = (td.x >> 8) & 7, sx = (oct & 1) ? -1 : 1;
+                const bool newtab = have && oct != taboct;       // this row's octant tables are not in shared memory yet
+                if (newtab) { taboct = oct; tabslot = (tabslot + 1) % kRowTabRing; }
                 for (int i = 0; i < nb; ++i, ++c) {
                     RowDesc d;
                     d.prob = td.x & 0xff; d.oct = oct; d.bj = td.y & 0x3ff; d.bk = (td.y >> 10) & 0x3ff;
                     d.bi = sx > 0 ? i : P.gbx - 1 - i;
-                    d.first = i == 0; d.last = i == nb - 1; d.stop = have ? 0 : 1;
+                    d.first = i == 0; d.last = i == nb - 1; d.stop = have ? 0 : 1; d.tab = tabslot;
                     sDesc[c % kRowRing] = d;
                     __threadfence_block();
                     sts_volatile_s32(leadAddr, c + 1);
@@ -213,9 +220,11 @@ k_sweep_row(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
                     }
                     if (have) {
                         const int brick = d.bi + P.gbx * (d.bj + P.gby * d.bk);
-                        mbar_expect_tx(bar_of(kBarQ, st), uint32_t(NM * NC * 4 + NC * 8));
+                        const bool tl = newtab && i == 0;          // the tables ride on the first brick's tile barrier
+                        mbar_expect_tx(bar_of(kBarQ, st), uint32_t(NM * NC * 4 + NC * 8 + (tl ? T.total : 0)));
                         tma_load_4d(tile_of(st), &tmQ, bar_of(kBarQ, st), 0, P.tm_rows * brick, 0, d.prob);
                         bulk_load(sig_of(st), P.sigt + (size_t)brick * P.NCb, uint32_t(NC * 8), bar_of(kBarQ, st));
+                        if (tl) bulk_load(smem_u32(tab_of(tabslot)), P.octtab + (size_t)oct * T.total, uint32_t(T.total), bar_of(kBarQ, st));
                     }
                 }
                 more = have;
@@ -235,20 +244,19 @@ k_sweep_row(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
             bulk_wait0();
             RT_FLUSH(0, true);
         }
-    } else if (warp == ctlW0 + 1 || warp == ctlW0 + 2) {
-        // ---- pollers (one warp per axis: y, z): inflow faces of every brick of the stream ----
-        const bool isz = warp == ctlW0 + 2;
-        for (int c = 0;; ++c) {
-            const RowDesc d = desc_at(c);
-            if (d.stop) break;
-            const int st = c % kRowStages;
-            if (c >= kRowStages) { RT_BEGIN; mbar_wait(bar_of(kBarFaceFree, st), uint32_t(c / kRowStages - 1) & 1u); RT_END(1); }
-            const int sy = (d.oct & 2) ? -1 : 1, sz = (d.oct & 4) ? -1 : 1;
-            const bool up = isz ? (sz > 0 ? d.bk > 0 : d.bk < P.gbz - 1) : (sy > 0 ? d.bj > 0 : d.bj < P.gby - 1);
-            const uint32_t dst = isz ? facez_of(st) : facey_of(st);
-            const int n8 = isz ? faceZn : faceYn;
-            if (up) {
-                if (lane == 0) {
+        else if (lane == 1 || lane == 2) {
+            // ---- pollers (lane 1: y, lane 2: z): inflow faces of every brick of the stream ----
+            const bool isz = lane == 2;
+            for (int c = 0;; ++c) {
+                const RowDesc d = desc_at(c);
+                if (d.stop) break;
+                const int st = c % kRowStages;
+                if (c >= kRowStages) { RT_BEGIN; mbar_wait(bar_of(kBarFaceFree, st), uint32_t(c / kRowStages - 1) & 1u); RT_END(1); }
+                const int sy = (d.oct & 2) ? -1 : 1, sz = (d.oct & 4) ? -1 : 1;
+                const bool up = isz ? (sz > 0 ? d.bk > 0 : d.bk < P.gbz - 1) : (sy > 0 ? d.bj > 0 : d.bj < P.gby - 1);
+                const uint32_t dst = isz ? facez_of(st) : facey_of(st);
+                const int n8 = isz ? faceZn : faceYn;
+                if (up) {
                     const int brick = d.bi + P.gbx * (d.bj + P.gby * d.bk);
                     const int upb = isz ? brick - sz * P.gbx * P.gby : brick - sy * P.gbx;
                     const size_t po = (size_t)d.prob * 8 + d.oct;
@@ -259,19 +267,16 @@ k_sweep_row(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
                     fence_proxy_async_all();
                     mbar_expect_tx(bar_of(kBarFace, st), uint32_t(n8) * 8u);
                     bulk_load(dst, src, uint32_t(n8) * 8u, bar_of(kBarFace, st));
+                } else {
+                    for (int e = 0; e < n8; ++e) sts_f64(dst + 8u * e, 0.0);   // vacuum
+                    mbar_arrive(bar_of(kBarFace, st));
                 }
-            } else {
-                for (int e = lane; e < n8; e += 32) sts_f64(dst + 8u * e, 0.0);   // vacuum
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar_of(kBarFace, st));
             }
-            __syncwarp();
+            RT_FLUSH(4, isz);
         }
-        RT_FLUSH(4, lane == 0 && isz);
-    }
-    else if (warp == ctlW0 + 3) {
-        // ---- publisher (one lane): outflow faces of every brick -> global, then the brick's flag ----
-        if (lane == 0) {
+        else if (lane == 3) {
+            // ---- publisher (lane 3): outflow faces of every brick -> global, then the brick's flag ----
+            {
             for (int c = 0;; ++c) {
                 const RowDesc d = desc_at(c);
                 if (d.stop) break;
@@ -292,17 +297,17 @@ k_sweep_row(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
                     st_release_u32(P.flags + po * nbricks + d.bi + P.gbx * (d.bj + P.gby * d.bk), P.epoch);
                 }
             }
+            }
             RT_FLUSH(8, true);
         }
     } else if (warp >= projW0 && warp < ctlW0) {
         // ---- projection warps: phase 0 of brick c+2, phase 2 of brick c (a5) ----
-        constexpr int CPT = 4;
         const int pt = tid - 32 * projW0, pn = 32 * kRowProjWarps;
         auto phase0 = [&](int c, const RowDesc& d) {
             const int st = c % kRowStages;
             { RT_BEGIN; mbar_wait(bar_of(kBarQ, st), uint32_t(c / kRowStages) & 1u); RT_END(1); }
             float* sQ = reinterpret_cast<float*>(smem + L.tile + size_t(st) * tileBytes);
-            const float* sM = reinterpret_cast<const float*>(tab_of(d.oct) + T.t0);
+            const float* sM = reinterpret_cast<const float*>(tab_of(d.tab) + T.t0);
             for (int c0 = pt; c0 < NC; c0 += CPT * pn) {
                 int cc[CPT]; bool ok[CPT];
 #pragma unroll
@@ -354,7 +359,7 @@ k_sweep_row(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
             const int st = c % kRowStages;
             { RT_BEGIN; mbar_wait(bar_of(kBarWave, st), uint32_t(c / kRowStages) & 1u); RT_END(2); }
             float* sQ = reinterpret_cast<float*>(smem + L.tile + size_t(st) * tileBytes);
-            const float* sD = reinterpret_cast<const float*>(tab_of(d.oct) + T.t2);
+            const float* sD = reinterpret_cast<const float*>(tab_of(d.tab) + T.t2);
             for (int c0 = pt; c0 < NC; c0 += CPT * pn) {
                 int cc[CPT]; bool ok[CPT];
 #pragma unroll
@@ -447,9 +452,11 @@ k_sweep_row(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
             const bool first_y = jp == 0, first_z = kp == 0, last_y = jp == ey - 1, last_z = kp == ez - 1;
             const bool edge_y = sy > 0 ? d0.bj == P.gby - 1 : d0.bj == 0;   // outflow faces on the mesh boundary
             const bool edge_z = sz > 0 ? d0.bk == P.gbz - 1 : d0.bk == 0;
-            const double* dir = reinterpret_cast<const double*>(tab_of(oct) + T.dir) + 4 * n;
+            // the octant's tables ride on the tile barrier of the row's first brick (one phase ahead at most: safe to wait here)
+            mbar_wait(bar_of(kBarQ, c % kRowStages), uint32_t(c / kRowStages) & 1u);
+            const double* dir = reinterpret_cast<const double*>(tab_of(d0.tab) + T.dir) + 4 * n;
             const double cx = dir[0], cy = dir[1], cz = dir[2], cs = dir[3];
-            const float4 lkc = reinterpret_cast<const float4*>(tab_of(oct) + T.lk)[n];
+            const float4 lkc = reinterpret_cast<const float4*>(tab_of(d0.tab) + T.lk)[n];
             int nxr = P.nx, gbx = P.gbx;
             asm volatile("" : "+r"(nxr), "+r"(gbx));             // kept in registers: otherwise re-read from the constant bank every step
             auto len_of = [&](int i) { return (sx > 0 ? i : gbx - 1 - i) == gbx - 1 ? exLast : BX; };
