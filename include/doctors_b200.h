@@ -51,6 +51,10 @@ typedef struct doctors_problem doctors_problem;
 /* Library version string, e.g. "doctors-b200 0.1 (sm_100a)". */
 const char* doctors_version(void);
 
+/* sizeof(doctors_source), sizeof(doctors_solve_opts), sizeof(doctors_solve_info) as this library was compiled:
+ * out_sizes[3] (host).  A binding checks its own struct declarations against them. */
+void doctors_abi_sizes(int* out_sizes);
+
 /* Create / destroy a problem bound to `cuda_device` and to `stream` (a cudaStream_t passed as
  * void*, e.g. torch.cuda.current_stream().cuda_stream; NULL = the legacy default stream).
  * All kernels and copies of this handle are issued on that stream.

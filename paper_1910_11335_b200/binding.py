@@ -17,7 +17,7 @@ OK, INVALID_ARG, BAD_STATE, ALLOC, CUDA, NOT_CONVERGED, NOT_RETAINED = range(7)
 STATUS_NAMES = ["OK", "INVALID_ARG", "BAD_STATE", "ALLOC", "CUDA", "NOT_CONVERGED", "NOT_RETAINED"]
 
 EXPORTS = [
-    "doctors_version", "doctors_create_problem", "doctors_destroy_problem", "doctors_last_error",
+    "doctors_version", "doctors_abi_sizes", "doctors_create_problem", "doctors_destroy_problem", "doctors_last_error",
     "doctors_set_mesh_materials", "doctors_set_xs", "doctors_set_quadrature", "doctors_set_quadrature_points",
     "doctors_get_quadrature", "doctors_set_source", "doctors_n_problems", "doctors_workspace_bytes",
     "doctors_set_workspace", "doctors_solve", "doctors_get_flux_moments", "doctors_get_uncollided_flux",
@@ -69,6 +69,14 @@ def load_library():
     L = C.CDLL(LIB_PATH)
     vp, ip, dp, fp = C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_double), C.POINTER(C.c_float)
     L.doctors_version.restype = C.c_char_p
+    L.doctors_abi_sizes.argtypes = [C.POINTER(C.c_int)]
+    L.doctors_abi_sizes.restype = None
+    sizes = (C.c_int * 3)()
+    L.doctors_abi_sizes(sizes)
+    mine = (C.sizeof(CSource), C.sizeof(CSolveOpts), C.sizeof(CSolveInfo))
+    if tuple(sizes) != mine:
+        raise ImportError("libdoctors_b200.so was built from another include/doctors_b200.h: struct sizes %s, binding %s"
+                          % (tuple(sizes), mine))
     L.doctors_create_problem.argtypes = [C.c_int, vp, C.POINTER(vp)]
     L.doctors_destroy_problem.argtypes = [vp]
     L.doctors_destroy_problem.restype = None

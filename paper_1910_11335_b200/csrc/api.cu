@@ -262,6 +262,14 @@ extern "C" {
 
 const char* doctors_version(void) { return "doctors-b200 0.1 (sm_100a)"; }
 
+void doctors_abi_sizes(int* out_sizes)
+{
+    if (!out_sizes) return;
+    out_sizes[0] = int(sizeof(doctors_source));
+    out_sizes[1] = int(sizeof(doctors_solve_opts));
+    out_sizes[2] = int(sizeof(doctors_solve_info));
+}
+
 int doctors_create_problem(int cuda_device, void* stream, doctors_problem** out)
 {
     if (!out) return DOCTORS_INVALID_ARG;

@@ -37,6 +37,18 @@ def test_header_symbols_exported(pkg):
     assert sorted(pkg.EXPORTS) == syms
 
 
+def test_struct_layouts_match_the_library(pkg):
+    """The ctypes declarations of the binding and the structs the library was compiled with have the same sizes
+    (load_library refuses a mismatch), and the option / info fields added for the sweep kernels are there."""
+    L = pkg.load_library()
+    sizes = (ctypes.c_int * 3)()
+    L.doctors_abi_sizes(sizes)
+    from paper_1910_11335_b200 import binding
+    assert tuple(sizes) == (ctypes.sizeof(binding.CSource), ctypes.sizeof(binding.CSolveOpts), ctypes.sizeof(binding.CSolveInfo))
+    assert [f[0] for f in binding.CSolveOpts._fields_][-2:] == ["check_window", "projection"]
+    assert [f[0] for f in binding.CSolveInfo._fields_][-2:] == ["sweep_kernel", "projection_mtiles"]
+
+
 def test_version_and_no_device_error(pkg):
     L = pkg.load_library()
     assert b"sm_100a" in L.doctors_version()
