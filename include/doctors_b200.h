@@ -164,6 +164,15 @@ int doctors_get_flux_moments(doctors_problem* p, int problem, int group, int l_m
 /* Uncollided scalar flux of Eq. (4) for one SOURCE and group: out [nz][ny][nx] fp32. */
 int doctors_get_uncollided_flux(doctors_problem* p, int source, int group, float* out, int out_is_device);
 
+/* Post-processing hook ("a conversion of photon fluence to an absorbed dose"): a response per group folded
+ * with the scalar fluence of one PROBLEM on the device,
+ *   out[nz][ny][nx] = sum_g response[g] * (phi_00,g + (include_uncollided ? sum over the problem's sources of phi_u,g : 0)),
+ * fp64 accumulation over the groups, fp32 result.  response: [G] doubles (host, copied).  The collided flux alone is what
+ * the sweep computes; the total fluence of the first-collision method is collided + uncollided.
+ * Errors: BAD_STATE before a successful solve, INVALID_ARG for a bad problem index or NULL pointers. */
+int doctors_get_response(doctors_problem* p, int problem, const double* response, int include_uncollided,
+                         float* out, int out_is_device);
+
 /* Test hooks: the integer schedules the kernels consume (Eqs. 8-22, Table 1),
  * for the bit-exact check against the oracle.
  *   level 0: cells of the whole mesh in sub-sweep order (what sweep_mode 1 launches over)

@@ -316,3 +316,25 @@ def solve(wl, closure=0, fixed_iters=None, threads=None, keep_history=False, ord
     if keep_history:
         res["history"] = history
     return res
+
+
+def response(res, wl, problem, resp, include_uncollided=True):
+    """Post-processing hook ("conversion of photon fluence to an absorbed dose"): a response per
+    group folded with the scalar fluence of one problem of `res` = solve(wl, ...):
+        D(cell) = sum_g resp[g] * (phi_00,g(cell) + sum over the problem's sources of phi_u,g(cell)).
+    The total fluence of the first-collision method is collided + uncollided.  Written out as the
+    definition: one term per group, in group order, float64.  Pins (tests/test_oracle_sweep.py): a unit response returns
+    the group's fluence itself, linearity in the response, and in a mode-1 (summed sources) problem the uncollided part is
+    the sum over all sources."""
+    resp = np.asarray(resp, dtype=np.float64)
+    nsrc = len(wl.sources)
+    srcs = range(nsrc) if wl.mode == 1 else [problem]
+    out = np.zeros(res["phi"].shape[-1], dtype=np.float64)
+    for g in range(wl.G):
+        f = res["phi"][problem, g, 0].copy()
+        if include_uncollided:
+            for s_ in srcs:
+                f += res["phi_u"][s_, g]
+        out += resp[g] * f
+    return out
+

@@ -20,7 +20,7 @@ EXPORTS = [
     "doctors_version", "doctors_abi_sizes", "doctors_create_problem", "doctors_destroy_problem", "doctors_last_error",
     "doctors_set_mesh_materials", "doctors_set_xs", "doctors_set_quadrature", "doctors_set_quadrature_points",
     "doctors_get_quadrature", "doctors_set_source", "doctors_n_problems", "doctors_workspace_bytes",
-    "doctors_set_workspace", "doctors_solve", "doctors_get_flux_moments", "doctors_get_uncollided_flux",
+    "doctors_set_workspace", "doctors_solve", "doctors_get_flux_moments", "doctors_get_uncollided_flux", "doctors_get_response",
     "doctors_debug_schedule_dims", "doctors_debug_get_schedule", "doctors_debug_device_brick_steps", "doctors_wavefront_size", "doctors_debug_get_tables",
     "doctors_host_level_symmetric", "doctors_host_schedule", "doctors_host_projection_tables",
 ]
@@ -96,6 +96,7 @@ def load_library():
     L.doctors_solve.argtypes = [vp, C.POINTER(CSolveOpts), C.POINTER(CSolveInfo)]
     L.doctors_get_flux_moments.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp, C.c_int]
     L.doctors_get_uncollided_flux.argtypes = [vp, C.c_int, C.c_int, vp, C.c_int]
+    L.doctors_get_response.argtypes = [vp, C.c_int, dp, C.c_int, vp, C.c_int]
     L.doctors_debug_schedule_dims.argtypes = [vp, C.POINTER(CSolveOpts), C.c_int, ip]
     L.doctors_debug_get_schedule.argtypes = [vp, C.POINTER(CSolveOpts), C.c_int, C.c_int,
                                              C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
@@ -321,6 +322,16 @@ class Problem:
     def get_uncollided_flux(self, source, group):
         host = np.empty(self.shape, dtype=np.float32)
         self._check(self._L.doctors_get_uncollided_flux(self._h, source, group, C.c_void_p(host.ctypes.data), 0))
+        return host
+
+    def get_response(self, problem, response, include_uncollided=True):
+        """doctors_get_response: sum_g response[g] * fluence_g of one problem, dense [nz][ny][nx] fp32."""
+        r = np.ascontiguousarray(response, dtype=np.float64)
+        if r.shape != (self.G,):
+            raise ValueError("response must have G = %d entries" % self.G)
+        host = np.empty(self.shape, dtype=np.float32)
+        self._check(self._L.doctors_get_response(self._h, problem, _ptr(r, C.c_double), int(bool(include_uncollided)),
+                                                 C.c_void_p(host.ctypes.data), 0))
         return host
 
     # ---- test hooks -------------------------------------------------------------------------

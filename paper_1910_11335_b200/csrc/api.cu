@@ -49,7 +49,7 @@ struct Plan {
     // offsets
     size_t o_mat, o_rho, o_sigt_hat, o_sigs, o_spec, o_srcs, o_extvol, o_mtab, o_dtab, o_lk,
         o_sigt, o_Q, o_fixed, o_phi0old, o_phiall, o_phi0all, o_phiu, o_state, o_ctl, o_leak, o_bal,
-        o_matd, o_rhod, o_scratch, o_results, o_fixediters, o_tasks, o_flags, o_fx, o_fy, o_fz, o_dird, o_dbg, o_sched, o_ox, o_oy, o_oz, o_octtab;
+        o_matd, o_rhod, o_scratch, o_results, o_fixediters, o_tasks, o_flags, o_fx, o_fy, o_fz, o_dird, o_dbg, o_sched, o_ox, o_oy, o_oz, o_octtab, o_resp;
     size_t face_x_n = 0, face_y_n = 0, face_z_n = 0;
     size_t total = 0;
 };
@@ -199,6 +199,7 @@ Plan make_plan(const doctors_problem* p, const doctors_solve_opts* o, int chunk)
     P.o_bal = take(size_t(P.chunk) * 16);
     P.o_results = take(size_t(P.nprob) * G * sizeof(GroupResult));
     P.o_fixediters = take(size_t(P.nprob) * G * 4);
+    P.o_resp = take(G * 8);
     if (P.sweep_mode == 0) {
         P.face_x_n = size_t(P.M) * P.B[1] * P.B[2];
         P.face_y_n = size_t(P.M) * P.B[0] * P.B[2];
@@ -1266,6 +1267,34 @@ extern "C" int doctors_get_flux_moments(doctors_problem* p, int problem, int gro
     const int nmo = (l_max + 1) * (l_max + 1);
     const float* src = at<float>(p, P.o_phiall) + ((size_t)q * P.G + group) * P.NM * cp;
     return copy_rows_out(p, src, out, out_is_device, nmo);
+}
+
+extern "C" int doctors_get_response(doctors_problem* p, int problem, const double* response, int include_uncollided,
+                                    float* out, int out_is_device)
+{
+    if (!p || !out || !response) return DOCTORS_INVALID_ARG;
+    if (!p->solved) return fail(p, DOCTORS_BAD_STATE, "no successful solve yet");
+    const Plan& P = p->plan;
+    if (problem < 0 || problem >= P.nprob) return fail(p, DOCTORS_INVALID_ARG, "bad problem");
+    cudaSetDevice(p->device);
+    const size_t cp = size_t(P.cells_p), n = size_t(p->nx) * p->ny * p->nz;
+    double* d_resp = at<double>(p, P.o_resp);
+    cudaError_t e = cudaMemcpyAsync(d_resp, response, size_t(P.G) * 8, cudaMemcpyHostToDevice, p->stream);
+    // mode 0: problem q is source q; mode 1: the one problem sums all sources
+    const int src0 = P.mode == 0 ? problem : 0, nsrc = P.mode == 0 ? 1 : P.nsrc;
+    bool any_unc = false;
+    for (int s_ = src0; s_ < src0 + nsrc; ++s_) if (p->sources[size_t(s_)].kind != 0) any_unc = true;
+    float* dst = out_is_device ? out : at<float>(p, P.o_scratch);
+    const int blocks = int(std::min<size_t>((n + 255) / 256, size_t(16) * p->num_sms));
+    if (e == cudaSuccess) {
+        k_response<<<blocks, 256, 0, p->stream>>>(p->mesh_dev, P.G, d_resp, at<float>(p, P.o_phi0all) + (size_t)problem * P.G * cp,
+                                                   (include_uncollided && any_unc) ? at<float>(p, P.o_phiu) : nullptr, src0, nsrc, dst);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess && !out_is_device) e = cudaMemcpyAsync(out, dst, n * 4, cudaMemcpyDeviceToHost, p->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
+    if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "response failed: %s", cudaGetErrorString(e));
+    return DOCTORS_OK;
 }
 
 extern "C" int doctors_get_uncollided_flux(doctors_problem* p, int source, int group, float* out, int out_is_device)

@@ -414,4 +414,26 @@ k_unbrick(MeshDev m, const float* __restrict__ src /*[fields][cells_p]*/, float*
     }
 }
 
+// Post-processing hook ("conversion of photon fluence to an absorbed dose"): a user-supplied
+// response per group folded with the scalar fluence of one problem,
+//   out(cell) = sum_g R_g * (phi_00,g(cell) [+ sum over the problem's sources of phi_u,s,g(cell)]),
+// written dense [nz][ny][nx].  fp64 accumulation over the groups, one thread per cell, streaming reads.
+__global__ void __launch_bounds__(256)
+k_response(MeshDev m, int G, const double* __restrict__ resp /*[G]*/, const float* __restrict__ phi0 /*[G][cells_p] of the problem*/,
+           const float* __restrict__ phiu /*[sources][G][cells_p] or NULL*/, int src0, int nsrc, float* __restrict__ dst)
+{
+    const long long cells = (long long)m.nx * m.ny * m.nz;
+    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < cells; c += (long long)gridDim.x * blockDim.x) {
+        const int i = int(c % m.nx), j = int((c / m.nx) % m.ny), kk = int(c / ((long long)m.nx * m.ny));
+        const long long cp = cell_index(m, i, j, kk);
+        double acc = 0.0;
+        for (int g = 0; g < G; ++g) {
+            double f = (double)phi0[(size_t)g * m.cells_p + cp];
+            if (phiu) for (int sidx = src0; sidx < src0 + nsrc; ++sidx) f += (double)phiu[((size_t)sidx * G + g) * m.cells_p + cp];
+            acc = fma(resp[g], f, acc);
+        }
+        dst[c] = (float)acc;
+    }
+}
+
 }  // namespace doctors

@@ -5,6 +5,8 @@ relative error wherever phi > 1e-6 max(phi), per (problem, group), after the ora
 counts are replayed on the GPU (reading R10).  Closure per reading R2: configs 0-1 gated with both
 closures, configs 2-4 with closure 1.
 """
+import dataclasses
+
 import numpy as np
 import pytest
 
@@ -230,6 +232,30 @@ def test_summed_sources_mode1(pkg, orc):
     assert ref["iters"].shape == (1, wl.G)
     worst = compare_workload(wl, ref, closure=0)
     assert worst < TOL, worst
+
+
+def test_response_hook(pkg, orc):
+    """doctors_get_response (PAPER.md:149 post-processing: fluence -> dose-like quantity) against the oracle's definition,
+    independent problems and summed sources, with and without the uncollided part."""
+    from workloads import SourceSpec
+    wl = tiny_p3_case(nx=13, ny=9, nz=6, G=3, sn=8, L=3, seed=4)
+    src2 = [wl.sources[0], SourceSpec(kind=2, pos=(0.4, -12.0, 0.3), axis=(0.0, 1.0, 0.0), half_angle=np.deg2rad(30.0),
+                                      spectrum=np.full(wl.G, 1.0 / wl.G))]
+    resp = np.array([0.25, 1.5, 3.0])
+    shape = (wl.nz, wl.ny, wl.nx)
+    for mode in (0, 1):
+        w2 = dataclasses.replace(wl, sources=src2, mode=mode)
+        ref = orc.solve(w2, closure=1)
+        p, info = run_gpu(w2, closure=1, fixed_iters=ref["iters"])
+        for q in range(ref["iters"].shape[0]):
+            for unc in (True, False):
+                got = p.get_response(q, resp, include_uncollided=unc)
+                want = orc.response(ref, w2, q, resp, include_uncollided=unc).reshape(shape)
+                e, _ = masked_rel_err(got, want)
+                assert e < TOL, (mode, q, unc, e)
+        with pytest.raises(ValueError):
+            p.get_response(0, resp[:2])
+        p.close()
 
 
 def test_api_errors(pkg):

@@ -252,3 +252,28 @@ def test_infinite_medium_limit(orc, closure):
     assert abs(mid - 1.0 / 0.5) < 1e-2
     src, col, leak = res["balance"][0, 0]
     assert abs(src - col - leak) < 1e-12 * src
+
+
+def test_response_hook_definition(orc):
+    """orc.response against what fixes it: a unit response picks one group's total fluence, it is linear in the
+    response, and a mode-1 problem adds the uncollided flux of every source."""
+    from tests.parity_util import tiny_p3_case
+    from workloads import SourceSpec
+    wl = tiny_p3_case(nx=6, ny=5, nz=4, G=3, sn=4, L=1, seed=2)
+    res = orc.solve(wl, closure=1)
+    for g in range(wl.G):
+        e = np.zeros(wl.G); e[g] = 1.0
+        np.testing.assert_allclose(orc.response(res, wl, 0, e), res["phi"][0, g, 0] + res["phi_u"][0, g], rtol=1e-15)
+        np.testing.assert_allclose(orc.response(res, wl, 0, e, include_uncollided=False), res["phi"][0, g, 0], rtol=0)
+    r1, r2 = np.array([0.3, 1.7, 2.0]), np.array([1.0, -0.5, 0.25])
+    np.testing.assert_allclose(orc.response(res, wl, 0, 2.0 * r1 + r2),
+                               2.0 * orc.response(res, wl, 0, r1) + orc.response(res, wl, 0, r2), rtol=1e-13, atol=1e-300)
+    # summed sources: one problem, the uncollided part is the sum over both sources
+    src2 = [wl.sources[0], SourceSpec(kind=1, pos=(0.4, -9.0, 0.3), spectrum=np.full(wl.G, 1.0 / wl.G))]
+    import dataclasses
+    wl2 = dataclasses.replace(wl, sources=src2, mode=1)
+    res2 = orc.solve(wl2, closure=1)
+    ones = np.ones(wl.G)
+    want = res2["phi"][0, :, 0].sum(0) + res2["phi_u"].sum((0, 1))
+    np.testing.assert_allclose(orc.response(res2, wl2, 0, ones), want, rtol=1e-14)
+
