@@ -14,14 +14,14 @@
 //            in a register, the y and z faces are handed to lanes (j'+1,k') / (j',k'+1) by warp
 //            shuffles: no shared-memory traffic, no block barrier inside the wavefront.
 //
-// Per task:  bulk async copies (TMA unit) bring Q_lm [NM][brick] (fp32, one contiguous run per moment in
-// the brick-major layout), sigma_t [brick] (fp64) and, when the octant changes, the octant's table blob
-// into shared memory; phase 0 projects moments -> directions (q_n, a5) for the whole brick; the
-// wavefront phase applies the diamond-difference update (a4) in place (q_n -> psi_n), its face
-// recurrence in fp64; brick-to-brick faces go through global buffers (L2) guarded by release/acquire
-// flags; phase 2 projects directions -> moments (Eq. 3) for the whole brick and bulk reduce-adds
-// (cp.reduce.async.bulk .add.f32) add the tile into phi in L2 (so octants may touch a cell concurrently
-// — the paper's obstacle at PAPER.md:119).  The angular flux never leaves the SM.
+// Per task:  one tensor copy (TMA, 4-D box) brings the dense tile Q_lm [NM][brick] (fp32) into shared memory — with the
+// tensor-core projections, whose planes are padded, one 1-D bulk copy per moment plane instead —, 1-D bulk copies bring
+// sigma_t [brick] (fp64) and, when the CTA changes octant, the octant's table blob; phase 0 projects moments ->
+// directions (q_n, a5) for the whole brick; the wavefront phase applies the diamond-difference update (a4) in place
+// (q_n -> psi_n), its face recurrence in fp64; brick-to-brick faces go through global buffers (L2) guarded by
+// release/acquire flags; phase 2 projects directions -> moments (Eq. 3) for the whole brick and one tensor reduce-add
+// (cp.reduce.async.bulk.tensor .add.f32) adds the tile into phi in L2 (so octants may touch a cell concurrently — the
+// paper's obstacle at PAPER.md:119).  The angular flux never leaves the SM.
 //
 // Projections (a5), template parameter MT:
 //   MT = 0  plain FFMA2 loops (any NM, any M).
