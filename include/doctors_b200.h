@@ -92,12 +92,14 @@ int doctors_get_quadrature(const doctors_problem* p, int* n_dir, double* omega_x
 
 /* Source description (reading R12).  The mesh is centred on the origin. */
 typedef struct {
-    int kind;                 /* 0 isotropic volume source, 1 isotropic point, 2 cone (hard edge) */
-    double pos[3];            /* kinds 1, 2: source position, cm */
-    double axis[3];           /* kind 2: cone axis (need not be normalised) */
-    double half_angle_rad;    /* kind 2 */
-    const double* spectrum;   /* kinds 1, 2: [G] photons emitted per group */
+    int kind;                 /* 0 isotropic volume source, 1 isotropic point, 2 cone (hard edge), 3 fan (hard edges) */
+    double pos[3];            /* kinds 1, 2, 3: source position, cm */
+    double axis[3];           /* kinds 2, 3: beam axis (need not be normalised) */
+    double half_angle_rad;    /* kind 2: half angle of the cone; kind 3: half of the azimuthal angle the fan subtends IN its plane */
+    const double* spectrum;   /* kinds 1, 2, 3: [G] photons emitted per group */
     const float* volume;      /* kind 0: [G][nz][ny][nx] photons/cm^3, 4pi-integrated (host) */
+    double up[3];             /* kind 3: a vector out of the fan plane (not parallel to axis); the plane is spanned by axis and up x axis */
+    double half_angle2_rad;   /* kind 3: half of the polar angle the fan subtends OUT of its plane, in (0, pi/2] (R18) */
 } doctors_source;
 /* mode 0: the n sources are independent problems, solved batched.
  * mode 1: the n sources are summed into ONE problem (the paper's CT scan).

@@ -204,7 +204,7 @@ def sweep(nx, ny, nz, dx, dy, dz, sigt, Q, omega, w, Mtab, Dtab, closure=0, orde
 
 
 def raytrace(wl, src, want_areal=False, threads=None):
-    """phi_u [G][cells] for one point / cone source (Eq. 4; readings R11, R12)."""
+    """phi_u [G][cells] for one point / cone / fan source (Eq. 4; readings R11, R12, R18)."""
     cells = wl.cells
     phi_u = np.zeros((wl.G, cells))
     areal = np.zeros((wl.n_materials, cells)) if want_areal else None
@@ -213,12 +213,20 @@ def raytrace(wl, src, want_areal=False, threads=None):
     pos = np.array(src.pos, dtype=np.float64)
     axis = np.array(src.axis, dtype=np.float64)
     spec = np.ascontiguousarray(src.spectrum, dtype=np.float64)
+    fan_n, sin_half2 = np.zeros(3), 0.0
+    if src.kind == 3:
+        # unit normal of the fan plane: the part of `up` perpendicular to the beam axis
+        a = axis / np.linalg.norm(axis)
+        up = np.array(src.up, dtype=np.float64)
+        fan_n = up - np.dot(up, a) * a
+        fan_n = fan_n / np.linalg.norm(fan_n)
+        sin_half2 = math.sin(src.half_angle2)
     _lib().orc_raytrace(wl.nx, wl.ny, wl.nz, ctypes.c_double(wl.dx), ctypes.c_double(wl.dy), ctypes.c_double(wl.dz),
                         _p(mat, ctypes.c_uint8), _p(rho), wl.n_materials, wl.G,
                         _p(np.ascontiguousarray(wl.sigma_t, dtype=np.float64)),
                         src.kind, _p(pos), _p(axis), ctypes.c_double(math.cos(src.half_angle)),
                         _p(spec), _p(phi_u), _p(areal) if want_areal else None,
-                        threads or default_threads())
+                        threads or default_threads(), _p(np.ascontiguousarray(fan_n)), ctypes.c_double(sin_half2))
     return (phi_u, areal) if want_areal else phi_u
 
 
@@ -261,7 +269,7 @@ def solve(wl, closure=0, fixed_iters=None, threads=None, keep_history=False, ord
     phi_u = np.zeros((n_src, G, cells))
     Yu = [None] * n_src
     for s, src in enumerate(wl.sources):
-        if src.kind in (1, 2):
+        if src.kind in (1, 2, 3):
             phi_u[s] = raytrace(wl, src, threads=threads)
             Yu[s] = real_sph_harm(L, unit_dirs_from(wl, src.pos)).T.copy()        # [nm][cells]
 

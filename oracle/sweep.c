@@ -229,6 +229,11 @@ void orc_sweep(int nx, int ny, int nz, double dx, double dy, double dz,
 /* ---- PAPER.md:44-49 Eq. (4): uncollided fluence by ray tracing (reading R11, R12) ----
  * For every cell centre r_c:  d = r_c - r_s, R = |d|, u = d/R.
  *   kind 2 (cone): u . axis >= cos_half, else phi_u = 0.
+ *   kind 3 (fan, "two additional parameters, phi and theta, describe the azimuthal and polar
+ *   angles subtended by the fan"; reading R18): with a = axis / |axis|, n = fan_n (unit normal of the fan plane,
+ *   perpendicular to a) and t = n x a, the direction u has the polar angle beta = asin(u . n) out of the plane
+ *   and the azimuth alpha = atan2(u . t, u . a) in it; lit iff |beta| <= half2 and |alpha| <= half, i.e.
+ *   |u . n| <= sin_half2 and u . a >= cos_half * sqrt((u . a)^2 + (u . t)^2).  Hard edges, 4 pi kept (R12).
  *   The segment [0,R] is clipped to the mesh box (outside is vacuum) and walked voxel by
  *   voxel (parametric traversal: per axis the next boundary crossing tMax and the step
  *   tDelta; always step the axis with the smallest tMax).  Per material m the areal
@@ -238,7 +243,8 @@ void orc_sweep(int nx, int ny, int nz, double dx, double dy, double dz,
 void orc_raytrace(int nx, int ny, int nz, double dx, double dy, double dz,
                   const uint8_t *mat, const double *rho, int n_mat, int G, const double *sigt_hat,
                   int kind, const double *spos, const double *axis, double cos_half,
-                  const double *spectrum, double *phi_u, double *areal, int nthreads)
+                  const double *spectrum, double *phi_u, double *areal, int nthreads,
+                  const double *fan_n, double sin_half2)
 {
     size_t cells = (size_t)nx * ny * nz;
     int nn[3] = {nx, ny, nz};
@@ -260,6 +266,15 @@ void orc_raytrace(int nx, int ny, int nz, double dx, double dy, double dz,
         if (kind == 2) {
             double ca = (u[0] * axis[0] + u[1] * axis[1] + u[2] * axis[2]) / an;
             if (ca < cos_half) lit = 0;
+        }
+        if (kind == 3) {
+            double a[3] = {axis[0] / an, axis[1] / an, axis[2] / an};
+            double t[3] = {fan_n[1] * a[2] - fan_n[2] * a[1], fan_n[2] * a[0] - fan_n[0] * a[2], fan_n[0] * a[1] - fan_n[1] * a[0]};
+            double ua = u[0] * a[0] + u[1] * a[1] + u[2] * a[2];
+            double un = u[0] * fan_n[0] + u[1] * fan_n[1] + u[2] * fan_n[2];
+            double ut = u[0] * t[0] + u[1] * t[1] + u[2] * t[2];
+            if (fabs(un) > sin_half2) lit = 0;
+            if (ua < cos_half * sqrt(ua * ua + ut * ut)) lit = 0;
         }
         if (lit) {
             /* clip [0,R] to the box: entry parameter */

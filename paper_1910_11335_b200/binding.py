@@ -35,7 +35,7 @@ class DoctorsError(RuntimeError):
 class CSource(C.Structure):
     _fields_ = [("kind", C.c_int), ("pos", C.c_double * 3), ("axis", C.c_double * 3),
                 ("half_angle_rad", C.c_double), ("spectrum", C.POINTER(C.c_double)),
-                ("volume", C.POINTER(C.c_float))]
+                ("volume", C.POINTER(C.c_float)), ("up", C.c_double * 3), ("half_angle2_rad", C.c_double)]
 
 
 class CSolveOpts(C.Structure):
@@ -235,6 +235,8 @@ class Problem:
             arr[i].pos = (C.c_double * 3)(*[float(v) for v in s.pos])
             arr[i].axis = (C.c_double * 3)(*[float(v) for v in s.axis])
             arr[i].half_angle_rad = float(s.half_angle)
+            arr[i].up = (C.c_double * 3)(*[float(v) for v in getattr(s, "up", (0.0, 0.0, 1.0))])
+            arr[i].half_angle2_rad = float(getattr(s, "half_angle2", 0.0))
             if s.spectrum is not None:
                 sp = np.ascontiguousarray(s.spectrum, dtype=np.float64)
                 keep.append(sp)

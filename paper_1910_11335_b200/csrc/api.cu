@@ -25,6 +25,7 @@ namespace {
 struct SourceHost {
     int kind = 0;
     double pos[3] = {0, 0, 0}, axis[3] = {1, 0, 0}, half = 0;
+    double fan_n[3] = {0, 0, 1}, half2 = 0;
     std::vector<double> spectrum;
     std::vector<float> volume;
 };
@@ -424,15 +425,27 @@ int doctors_set_source(doctors_problem* p, int n_sources, const doctors_source* 
             if (!S.volume) return fail(p, DOCTORS_INVALID_ARG, "source %d: volume is NULL", s);
             H.volume.assign(S.volume, S.volume + size_t(p->G) * cells);
             for (float f : H.volume) if (!std::isfinite(f)) return fail(p, DOCTORS_INVALID_ARG, "source %d: volume not finite", s);
-        } else if (S.kind == 1 || S.kind == 2) {
+        } else if (S.kind == 1 || S.kind == 2 || S.kind == 3) {
             if (!S.spectrum) return fail(p, DOCTORS_INVALID_ARG, "source %d: spectrum is NULL", s);
             H.spectrum.assign(S.spectrum, S.spectrum + p->G);
             for (int a = 0; a < 3; ++a) { H.pos[a] = S.pos[a]; H.axis[a] = S.axis[a]; }
             H.half = S.half_angle_rad;
-            if (S.kind == 2) {
+            if (S.kind == 2 || S.kind == 3) {
                 double an = std::sqrt(S.axis[0] * S.axis[0] + S.axis[1] * S.axis[1] + S.axis[2] * S.axis[2]);
-                if (!(an > 0.0) || !(S.half_angle_rad > 0.0)) return fail(p, DOCTORS_INVALID_ARG, "source %d: cone needs an axis and a half angle", s);
+                if (!(an > 0.0) || !(S.half_angle_rad > 0.0)) return fail(p, DOCTORS_INVALID_ARG, "source %d: cone / fan needs an axis and a half angle", s);
                 for (int a = 0; a < 3; ++a) H.axis[a] = S.axis[a] / an;
+            }
+            if (S.kind == 3) {
+                // normal of the fan plane: the part of `up` perpendicular to the axis
+                const double ua = S.up[0] * H.axis[0] + S.up[1] * H.axis[1] + S.up[2] * H.axis[2];
+                double nv[3], nn2 = 0.0;
+                for (int a = 0; a < 3; ++a) { nv[a] = S.up[a] - ua * H.axis[a]; nn2 += nv[a] * nv[a]; }
+                const double upn = S.up[0] * S.up[0] + S.up[1] * S.up[1] + S.up[2] * S.up[2];
+                if (!(nn2 > 1e-24 * upn) || !(upn > 0.0)) return fail(p, DOCTORS_INVALID_ARG, "source %d: fan needs an up vector that is not parallel to its axis", s);
+                if (!(S.half_angle2_rad > 0.0) || S.half_angle2_rad > 1.5707963267948968 || S.half_angle_rad > 3.1415926535897936)
+                    return fail(p, DOCTORS_INVALID_ARG, "source %d: fan angles: 0 < half_angle <= pi, 0 < half_angle2 <= pi/2", s);
+                for (int a = 0; a < 3; ++a) H.fan_n[a] = nv[a] / std::sqrt(nn2);
+                H.half2 = S.half_angle2_rad;
             }
             // 1/R^2 singularity: a source on a cell centre
             const double d[3] = {p->dx, p->dy, p->dz};
@@ -793,6 +806,8 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
             D.kind = H.kind; D.vol_slot = -1;
             for (int a = 0; a < 3; ++a) { D.pos[a] = H.pos[a]; D.axis[a] = H.axis[a]; }
             D.cos_half = std::cos(H.half);
+            for (int a = 0; a < 3; ++a) D.fan_n[a] = H.fan_n[a];
+            D.sin_half2 = std::sin(H.half2);
             if (H.kind == 0) {
                 D.vol_slot = slot;
                 std::vector<float> hv(size_t(G) * cp, 0.0f);

@@ -42,11 +42,13 @@ __host__ __device__ __forceinline__ bool cell_ijk(const MeshDev& m, long long cp
 }
 
 struct SourceDev {
-    int kind;               // 0 volume, 1 point, 2 cone
+    int kind;               // 0 volume, 1 point, 2 cone, 3 fan
     int vol_slot;           // kind 0: index into the volume-source array, else -1
     double pos[3];
     double axis[3];         // normalised
     double cos_half;
+    double fan_n[3];        // kind 3: unit normal of the fan plane (perpendicular to axis)
+    double sin_half2;       // kind 3: sine of the polar half angle
 };
 
 // Per-problem iteration state, device resident (row a6).

@@ -46,6 +46,14 @@ k_raytrace(MeshDev m, const uint8_t* __restrict__ mat /*dense [nz][ny][nx]*/, co
     for (int a = 0; a < 3; ++a) u[a] = d[a] / R;
     bool lit = true;
     if (src.kind == 2) lit = (u[0] * src.axis[0] + u[1] * src.axis[1] + u[2] * src.axis[2]) >= src.cos_half;
+    if (src.kind == 3) {
+        // fan beam (reading R18): polar angle out of the fan plane |beta| <= half2, azimuth in the plane |alpha| <= half
+        const double* a = src.axis; const double* nv = src.fan_n;
+        const double tv[3] = {nv[1] * a[2] - nv[2] * a[1], nv[2] * a[0] - nv[0] * a[2], nv[0] * a[1] - nv[1] * a[0]};
+        const double ua = u[0] * a[0] + u[1] * a[1] + u[2] * a[2], un = u[0] * nv[0] + u[1] * nv[1] + u[2] * nv[2];
+        const double ut = u[0] * tv[0] + u[1] * tv[1] + u[2] * tv[2];
+        lit = fabs(un) <= src.sin_half2 && ua >= src.cos_half * sqrt(ua * ua + ut * ut);
+    }
     if (lit) {
         double t0 = 0.0;                                 // entry parameter of the box
 #pragma unroll

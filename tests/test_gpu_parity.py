@@ -234,6 +234,27 @@ def test_summed_sources_mode1(pkg, orc):
     assert worst < TOL, worst
 
 
+def test_fan_beam_source(pkg, orc):
+    """Source kind 3 (fan beam, reading R18): uncollided and collided flux against the oracle, a fan
+    tilted against every mesh axis so that all three direction cosines enter the mask; bad fans are refused."""
+    from workloads import SourceSpec
+    wl = tiny_p3_case(nx=13, ny=11, nz=9, G=2, sn=8, L=3, seed=6)
+    fan = SourceSpec(kind=3, pos=(-11.0, 2.0, 1.5), axis=(1.0, -0.15, -0.1), up=(0.1, 0.3, 1.0), half_angle=np.deg2rad(24.0),
+                     half_angle2=np.deg2rad(9.0), spectrum=np.full(wl.G, 1.0 / wl.G))
+    w2 = dataclasses.replace(wl, sources=[fan])
+    ref = orc.solve(w2, closure=1)
+    lit = (ref["phi_u"][0, 0] > 0).mean()
+    assert 0.05 < lit < 0.9                                      # a real mask: some cells lit, some dark
+    worst = compare_workload(w2, ref, closure=1)
+    assert worst < TOL, worst
+    p = pkg.problem_from_workload(w2)
+    for bad in (dataclasses.replace(fan, up=(2.0, -0.3, -0.2)), dataclasses.replace(fan, half_angle2=0.0),
+                dataclasses.replace(fan, half_angle2=2.0)):
+        with pytest.raises(pkg.DoctorsError):
+            p.set_source([bad], 0)
+    p.close()
+
+
 def test_response_hook(pkg, orc):
     """doctors_get_response (PAPER.md:149 post-processing: fluence -> dose-like quantity) against the oracle's definition,
     independent problems and summed sources, with and without the uncollided part."""

@@ -65,6 +65,47 @@ def test_cone_mask(orc):
     assert np.array_equal(b[0][inside], a[0][inside]) and (b[0][~inside] == 0).all()   # hard edge, 4 pi kept (R12)
 
 
+def test_fan_mask(orc):
+    """Fan beam (reading R18) pinned by geometry the formula does not contain: the full fan is the
+    point source; the lit set is the set of cells whose angles, measured independently with arctan2 / arcsin in a frame
+    built by hand for this axis, lie inside the two openings; it is mirror-symmetric about the fan plane and about the
+    plane through the axis perpendicular to it; a thin fan lights a slab, a narrow one a wedge; lit values keep the 4 pi."""
+    wl = _homog(12, 12, 10, (1.0, 1.0, 1.0), 1.0, 0.1, G=1)
+    pos = (-20.0, 0.0, 0.0)
+    one = np.array([1.0])
+    point = orc.raytrace(wl, SourceSpec(kind=1, pos=pos, spectrum=one))[0]
+    full = orc.raytrace(wl, SourceSpec(kind=3, pos=pos, axis=(1.0, 0.0, 0.0), up=(0.0, 0.0, 1.0), half_angle=math.pi,
+                                      half_angle2=math.pi / 2, spectrum=one))[0]
+    assert np.array_equal(full, point)
+    half, half2 = math.radians(11.0), math.radians(4.0)
+    fan = orc.raytrace(wl, SourceSpec(kind=3, pos=pos, axis=(3.0, 0.0, 0.0), up=(0.2, 0.0, 5.0), half_angle=half,
+                                     half_angle2=half2, spectrum=one))[0]
+    # axis = +x, fan plane = x-y (up's component along the axis does not matter), so: azimuth = atan2(u_y, u_x), polar = asin(u_z)
+    u = orc.unit_dirs_from(wl, pos)
+    alpha, beta = np.arctan2(u[:, 1], u[:, 0]), np.arcsin(u[:, 2])
+    eps = 1e-12
+    surely_in = (np.abs(alpha) < half - eps) & (np.abs(beta) < half2 - eps)
+    surely_out = (np.abs(alpha) > half + eps) | (np.abs(beta) > half2 + eps)
+    assert 0 < surely_in.sum() < u.shape[0] and (surely_in | surely_out).all()
+    assert np.array_equal(fan[surely_in], point[surely_in]) and (fan[surely_out] == 0).all()
+    f3 = fan.reshape(wl.nz, wl.ny, wl.nx)
+    # mirror in z (the fan plane) and in y: the same cells are lit, with the same values up to the rounding of the traversal
+    assert np.array_equal(f3 > 0, f3[::-1] > 0) and np.array_equal(f3 > 0, f3[:, ::-1] > 0)
+    np.testing.assert_allclose(f3, f3[::-1], rtol=1e-13)
+    np.testing.assert_allclose(f3, f3[:, ::-1], rtol=1e-13)
+    # a thin fan is a slab around z = 0, a fan that is wide in its plane and thin out of it covers every y of that slab
+    lit = f3 > 0
+    assert lit[wl.nz // 2 - 1: wl.nz // 2 + 1].any() and not lit[0].any() and not lit[-1].any()
+    wide = orc.raytrace(wl, SourceSpec(kind=3, pos=pos, axis=(1.0, 0.0, 0.0), up=(0.0, 0.0, 1.0), half_angle=math.radians(60.0),
+                                      half_angle2=half2, spectrum=one))[0].reshape(wl.nz, wl.ny, wl.nx)
+    assert (wide[wl.nz // 2] > 0).all() and ((wide > 0) >= lit).all()
+    # rotating the frame rotates the pattern: fan plane x-z instead of x-y
+    rot = orc.raytrace(_homog(12, 10, 12, (1.0, 1.0, 1.0), 1.0, 0.1, G=1),
+                       SourceSpec(kind=3, pos=pos, axis=(1.0, 0.0, 0.0), up=(0.0, 1.0, 0.0), half_angle=half, half_angle2=half2,
+                                  spectrum=one))[0].reshape(12, 10, 12)
+    np.testing.assert_allclose(rot, f3.transpose(1, 0, 2), rtol=1e-13)
+
+
 def test_heterogeneous_against_brute_force_sampling(orc):
     """Optical depth through the config-1 sphere phantom vs a dumb midpoint-rule path integral."""
     wl = make_config(1)

@@ -21,12 +21,14 @@ B0 = np.array([0.1605, 0.1605, 0.1605, 0.170])       # cm^2/g        (scatter-li
 
 @dataclass
 class SourceSpec:
-    kind: int                       # 0 volume (isotropic), 1 point (isotropic), 2 cone
+    kind: int                       # 0 volume (isotropic), 1 point (isotropic), 2 cone, 3 fan
     pos: tuple = (0.0, 0.0, 0.0)
     axis: tuple = (1.0, 0.0, 0.0)
-    half_angle: float = 0.0         # radians (kind 2)
-    spectrum: np.ndarray = None     # [G] photons per group (kinds 1, 2)
+    half_angle: float = 0.0         # radians (kind 2: cone half angle; kind 3: azimuthal half angle in the fan plane)
+    spectrum: np.ndarray = None     # [G] photons per group (kinds 1, 2, 3)
     volume: np.ndarray = None       # [G][nz][ny][nx] float32 photons/cm^3 (kind 0)
+    up: tuple = (0.0, 0.0, 1.0)     # kind 3: a vector out of the fan plane
+    half_angle2: float = 0.0        # kind 3: polar half angle out of the fan plane
 
 
 @dataclass
