@@ -315,16 +315,16 @@ template <bool FIX>
 __device__ __forceinline__ float dd_cell(bool act, float q, double sig, double cx, double cy, double cz, double csum,
                                          double a, double b, double c, double& ox, double& oy, double& oz)
 {
-    const double ta = cx * a, tb = cy * b, tc = cz * c;
+    // numerator as an FMA chain (the late arrivals b, c enter last: two dependent FMAs instead of multiply + two adds)
     const double dq = (double)q;
-    double psi = (dq + ta + tb + tc) * rcp_f64(sig + csum);
+    double psi = fma(cz, c, fma(cy, b, fma(cx, a, dq))) * rcp_f64(sig + csum);
     ox = fma(2.0, psi, -a);
     oy = fma(2.0, psi, -b);
     oz = fma(2.0, psi, -c);
     if (FIX) {
         // any negative outflow?  (sign bits; -0.0 takes the slow path too, which then changes nothing)
         const int sgn = __double2hiint(ox) | __double2hiint(oy) | __double2hiint(oz);
-        if (act && sgn < 0) psi = dd_fixup(dq, sig, cx, cy, cz, ta, tb, tc, a, b, c, ox, oy, oz);
+        if (act && sgn < 0) psi = dd_fixup(dq, sig, cx, cy, cz, cx * a, cy * b, cz * c, a, b, c, ox, oy, oz);
     }
     return (float)psi;
 }
