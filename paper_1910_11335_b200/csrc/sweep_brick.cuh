@@ -546,8 +546,11 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         // inside this CTA's shared memory, which starts with a 128-byte pad and ends with the tables — and
         // compute on that garbage; only stores and the x-face register are predicated.  Clipped lanes
         // (beyond ey / ez) stay parked on the tile's first cell.
-        const int d4 = lane_ok ? 4 * sx : 0, d8 = 2 * d4;
-        const int shy = BY;
+        int d4 = lane_ok ? 4 * sx : 0, d8 = 2 * d4;
+        int shy = BY, ly = last_y ? 1 : 0, lz = last_z ? 1 : 0;
+        // loop invariants pinned in registers: otherwise the compiler re-derives them every step (constant-bank reads,
+        // ey - 1 / ez - 1 on the uniform datapath, 2 * d4)
+        asm volatile("" : "+r"(d4), "+r"(d8), "+r"(shy), "+r"(ly), "+r"(lz));
         for (int n = warp; n < M; n += P.W) {
             const double cx = sDir[4 * n], cy = sDir[4 * n + 1], cz = sDir[4 * n + 2], cs = sDir[4 * n + 3];
             double* fxp = sFx + n * (BY * BZ) + lj + BY * lk_;
@@ -570,8 +573,8 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
                 double ox;
                 const float psi = dd_cell<FIX>(act, q, sg, cx, cy, cz, cs, ax, b, cc, ox, oy, oz);
                 sts_f32_if(act, pq, psi);
-                sts_f64_if(act && last_y, py, oy);
-                sts_f64_if(act && last_z, pz, oz);
+                sts_f64_if(act && ly, py, oy);
+                sts_f64_if(act && lz, pz, oz);
                 if (act) ax = ox;
                 if (DBG && act) P.dbg_plane[(pq - smem_u32(sPsi)) / 4u - uint32_t(n * NCP)] = nsteps - s;
                 ++ip; pq += d4; ps += d8; py += d8; pz += d8;
