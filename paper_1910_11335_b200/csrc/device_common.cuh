@@ -176,6 +176,8 @@ __device__ __forceinline__ void tma_store_5d(const CUtensorMap* map, uint32_t sr
         : "memory");
 }
 __device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
+// generic <-> async proxy ordering for GLOBAL memory only (flags vs bulk copies of the face buffers)
+__device__ __forceinline__ void fence_proxy_async_global() { asm volatile("fence.proxy.async.global;" ::: "memory"); }
 // 1-D bulk copies through the TMA unit (no tensor map): size and both addresses multiples of 16 bytes
 __device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar)
 {

@@ -367,7 +367,7 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
             // the other 31 lanes run ahead to the tile wait of the next task; this one joins them there
             if (lane == 31) {
                 bulk_wait0();                                    // the face blocks are in global memory
-                fence_proxy_async_all();
+                fence_proxy_async_global();
                 st_release_u32(pub_flag, P.epoch);
             }
             publish = false;
@@ -432,7 +432,7 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
                     const uint32_t dst = smem_u32(lane == 0 ? sFx : (lane == 1 ? sFy : sFz));
                     const uint32_t bytes = 8u * uint32_t(lane == 0 ? faceXn : (lane == 1 ? faceYn : faceZn));
                     while (ld_acquire_u32(flag_base + up) != P.epoch) { }
-                    fence_proxy_async_all();                     // flag acquired (generic proxy) -> async-proxy read of the face
+                    fence_proxy_async_global();                     // flag acquired (generic proxy) -> async-proxy read of the face
                     mbar_expect_tx(barF, bytes);
                     bulk_load(dst, src, bytes, barF);            // 1-D bulk copy (TMA unit); needed after phase 0
                 } else {
