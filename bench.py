@@ -239,6 +239,12 @@ def run_gpu_arm(args):
               fixed_iters=(wl.fixed_iters if wl.fixed_iters else None))
     if args.config == 4 and not args.slice:
         kw["source_chunk"] = 4               # 2 chunks of 4: all-group moments of 8 sources exceed HBM
+    if args.projection:
+        kw["projection"] = args.projection
+    if args.brick:
+        kw["brick"] = tuple(int(v) for v in args.brick.split(","))
+    if args.ctas:
+        kw["ctas_per_sm"] = args.ctas
     flush = None
     if wl.cells * 33 * 4 * min(4, len(wl.sources)) <= 126e6:
         flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
@@ -354,6 +360,9 @@ def main():
     ap.add_argument("--closure", type=int, default=1, help="0 pure diamond difference, 1 + set-to-zero fix-up (R2)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--slice", action="store_true", help="profiling slice of the config (see workload_for); not a bench number")
+    ap.add_argument("--projection", type=int, default=0, help="doctors_solve_opts.projection (experiments; 0 = the library's default)")
+    ap.add_argument("--brick", default="", help="bx,by,bz brick extents (experiments; default automatic)")
+    ap.add_argument("--ctas", type=int, default=0, help="persistent CTAs per SM (experiments; default occupancy maximum)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--traffic", type=float, default=None,
