@@ -114,9 +114,8 @@ typedef struct {
     int closure;              /* 0 pure diamond difference; 1 + set-to-zero fix-up with rebalance (R2) */
     int deterministic;        /* 1: octants swept one after another, fixed summation order (bit-reproducible) */
     int source_chunk;         /* problems solved together (HBM capacity); 0 = all that fit the workspace */
-    int sweep_mode;           /* 0 brick wavefront kernel (product path); 1 the paper's one-launch-per-sub-sweep scheme;
-                               * 2 row-pipelined wavefront kernel (one CTA per SM sweeps x-rows of bricks) where it applies
-                               *   (<= 10 directions per octant, brick length >= BY + BZ - 2), else the brick kernel */
+    int sweep_mode;           /* 0 brick wavefront kernel (product path); 1 the paper's one-launch-per-sub-sweep scheme,
+                               * kept as a comparison arm */
     int brick[3];             /* sweep_mode 0: brick extents in cells; 0 = automatic.  brick[0] % 4 == 0, brick[1]*brick[2] <= 32 */
     int ctas_per_sm;          /* sweep_mode 0: persistent CTAs per SM; 0 = occupancy maximum */
     int check_window;         /* tolerance mode: sweeps enqueued between host reads of the device flag; 0 = adaptive
@@ -138,7 +137,7 @@ typedef struct {
     int n_chunks;
     int brick[3];
     int ctas_per_sm;
-    int sweep_kernel;         /* kernel that swept: 0 brick, 1 paper scheme, 2 row-pipelined */
+    int sweep_kernel;         /* kernel that swept: 0 brick, 1 paper scheme */
     int projection_mtiles;    /* > 0: the projections ran on the tensor cores (16-direction m-tiles per octant); 0: fp32 FMA loops */
 } doctors_solve_info;
 

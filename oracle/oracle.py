@@ -243,14 +243,21 @@ def unit_dirs_from(wl, pos):
 # --------------------------------------------------------------------------------------
 # Multigroup source iteration (PAPER.md:34 Eq. 2, :44-62 Eqs. 4-7, :149, :183)
 # --------------------------------------------------------------------------------------
-def solve(wl, closure=0, fixed_iters=None, threads=None, keep_history=False, order=0):
+def solve(wl, closure=0, fixed_iters=None, threads=None, keep_history=False, order=0, store_dtype=np.float64, progress=None):
     """Whole hot path for a Workload.  Returns a dict:
          phi     [n_prob][G][nm][cells]  collided flux moments (float64)
          phi_u   [n_src][G][cells]       uncollided scalar flux (zeros for kind 0)
          iters   [n_prob][G], residual [n_prob][G], balance [n_prob][G][3] (source, collision, leakage
                  of the LAST sweep: sum Q_00 V = sum sigt phi_0 V + leakage)
+         seconds dict: wall time spent in the ray trace, the fixed-source assembly and the sweeps (for bench.py)
        n_prob = n_src (mode 0) or 1 (mode 1, sources summed: linearity of Eq. 4-6).
-       fixed_iters: None -> wl.fixed_iters (0 = run to wl.tol); int or [n_prob][G] array -> replay."""
+       fixed_iters: None -> wl.fixed_iters (0 = run to wl.tol); int or [n_prob][G] array -> replay.
+       store_dtype: type in which the moments of FINISHED groups are held (they feed the downscatter source of the
+       groups below).  float64 everywhere except the config-4 goldens (tests/golden/make_goldens.py), where 47 groups
+       x 16 moments x 8.4 M cells would take 50 GB per source: float32 there (relative rounding 6e-8, three orders
+       below the 1e-4 gate; the iteration of the current group is always float64).
+       progress: None or a callable (problem, group, sweeps, delta) called after every finished group (logging only)."""
+    import time
     cells, G, L = wl.cells, wl.G, wl.L
     nm = (L + 1) ** 2
     ll = l_of_lm(L)
@@ -264,24 +271,30 @@ def solve(wl, closure=0, fixed_iters=None, threads=None, keep_history=False, ord
     if fixed_iters is None:
         fixed_iters = wl.fixed_iters
     fi = np.broadcast_to(np.asarray(fixed_iters), (len(probs), G))
+    seconds = dict(raytrace=0.0, fixed_source=0.0, sweep=0.0)
 
     # step 4: uncollided flux per source (Eq. 4) and its direction moments Y_lm(u_c)
+    t0 = time.perf_counter()
     phi_u = np.zeros((n_src, G, cells))
     Yu = [None] * n_src
     for s, src in enumerate(wl.sources):
         if src.kind in (1, 2, 3):
             phi_u[s] = raytrace(wl, src, threads=threads)
             Yu[s] = real_sph_harm(L, unit_dirs_from(wl, src.pos)).T.copy()        # [nm][cells]
+    seconds["raytrace"] = time.perf_counter() - t0
 
-    out_phi = np.zeros((len(probs), G, nm, cells))
+    out_phi = np.zeros((len(probs), G, nm, cells), dtype=store_dtype)
     iters = np.zeros((len(probs), G), dtype=np.int64)
     resid = np.zeros((len(probs), G))
     balance = np.zeros((len(probs), G, 3))
     history = [[[] for _ in range(G)] for _ in probs]
+    lm_of = [slice(l * l, (l + 1) * (l + 1)) for l in range(L + 1)]              # moments lm of degree l
     for p, members in enumerate(probs):
         for g in range(G):                                                      # high -> low energy (R7)
+            t0 = time.perf_counter()
             sigt = rho * wl.sigma_t[mat, g]
-            # step 5 / row a2: fixed source = external + first-collision (Eq. 5) + downscatter (Eq. 2 rhs, g' < g)
+            # step 5 / row a2: fixed source = external + first-collision (Eq. 5) + downscatter (Eq. 2 rhs, g' < g),
+            # moment lm of degree l:  rho(c) s_l[mat(c)][g' -> g] * {phi_u^{g'}(c) Y_lm(u_c)  |  phi_lm^{g'}(c)}
             fixed = np.zeros((nm, cells))
             for s in members:
                 src = wl.sources[s]
@@ -289,20 +302,24 @@ def solve(wl, closure=0, fixed_iters=None, threads=None, keep_history=False, ord
                     fixed[0] += np.asarray(src.volume[g], dtype=np.float64).reshape(-1)
                 else:
                     for gp in range(g + 1):
-                        ss = wl.sigma_s[:, :, gp, g][mat]                       # [cells][L+1]
-                        fixed += (rho * phi_u[s, gp])[None, :] * ss[:, ll].T * Yu[s]
+                        ru = rho * phi_u[s, gp]
+                        for l in range(L + 1):
+                            fixed[lm_of[l]] += (ru * wl.sigma_s[:, l, gp, g][mat])[None, :] * Yu[s][lm_of[l]]
             for gp in range(g):
-                ss = wl.sigma_s[:, :, gp, g][mat]
-                fixed += rho[None, :] * ss[:, ll].T * out_phi[p, gp]
+                for l in range(L + 1):
+                    fixed[lm_of[l]] += (rho * wl.sigma_s[:, l, gp, g][mat])[None, :] * out_phi[p, gp, lm_of[l]]
             s_self = rho[None, :] * wl.sigma_s[:, :, g, g][mat][:, ll].T          # [nm][cells]
+            seconds["fixed_source"] += time.perf_counter() - t0
             # step 6 / row a6: source iteration from phi = 0 (R9)
             phi = np.zeros((nm, cells))
             k = 0
             while True:
                 k += 1
                 Q = s_self * phi + fixed
+                t0 = time.perf_counter()
                 phi_new, leak, _, _ = sweep(wl.nx, wl.ny, wl.nz, wl.dx, wl.dy, wl.dz, sigt, Q,
                                             omega, w, Mtab, Dtab, closure, order, threads=threads)
+                seconds["sweep"] += time.perf_counter() - t0
                 mx = np.abs(phi_new[0]).max()
                 delta = 0.0 if mx == 0.0 else np.abs(phi_new[0] - phi[0]).max() / mx   # R8
                 phi = phi_new
@@ -319,8 +336,10 @@ def solve(wl, closure=0, fixed_iters=None, threads=None, keep_history=False, ord
             iters[p, g] = k
             resid[p, g] = delta
             balance[p, g] = (Q[0].sum() * V, (sigt * phi[0]).sum() * V, leak)
+            if progress is not None:
+                progress(p, g, k, delta)
     res = dict(phi=out_phi, phi_u=phi_u, iters=iters, residual=resid, balance=balance,
-               omega=omega, w=w)
+               omega=omega, w=w, seconds=seconds)
     if keep_history:
         res["history"] = history
     return res

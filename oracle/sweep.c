@@ -174,8 +174,11 @@ static double sweep_dir_hyperplane(int nx, int ny, int nz, const double del[3], 
  * Q    [nm][cells]  source moments (4pi-integrated convention, reading R6)
  * Mtab [ndir][nm]   (2l+1)/(4pi) Y_lm(Omega_n)       -> q_n = sum_lm Mtab[n][lm] Q_lm   (Eq. 2 rhs, moment form R3)
  * Dtab [nm][ndir]   w_n Y_lm(Omega_n)                -> phi_lm += Dtab[lm][n] psi_n     (Eq. 3)
- * Directions are ordered octant-major (octant o = n / (ndir/8)); they are processed
- * octant by octant, directions of the octant in index order, and summed in that order.
+ * Directions are ordered octant-major (octant o = n / (ndir/8)).  Every direction is independent of the others
+ * (PAPER.md:119 discusses exactly this), so they are computed in batches of whole octants, one thread per
+ * direction; phi_lm(c) is then summed over the directions of the batch in index order, batches in order: for
+ * every (lm, c) the terms are added in the order n = 0, 1, ..., ndir-1 whatever the batch size and the
+ * thread count are (the batch only bounds the memory held for psi_n: 6 GiB).
  * order: 0 lexicographic loops, 1 the paper's sub-sweep order.
  * psi_all: NULL or [ndir][cells] (angular flux, for tests).
  * leak_out: sum_n w_n * leakage_n.   nfix_out: NULL or fix-up event count. */
@@ -188,16 +191,21 @@ void orc_sweep(int nx, int ny, int nz, double dx, double dy, double dz,
 {
     size_t cells = (size_t)nx * ny * nz;
     double del[3] = {dx, dy, dz};
-    int chunk = ndir / 8 > 0 && ndir % 8 == 0 ? ndir / 8 : ndir;   /* directions summed per batch */
+    int per_oct = ndir / 8 > 0 && ndir % 8 == 0 ? ndir / 8 : ndir;
+    int chunk = per_oct;                                            /* directions per batch: whole octants */
+    while (chunk + per_oct <= ndir && (double)cells * (chunk + per_oct) * 16.0 <= 6.0 * 1073741824.0) chunk += per_oct;
     double *psi_buf = (double *)malloc(sizeof(double) * cells * chunk);
     double *qn_buf = (double *)malloc(sizeof(double) * cells * chunk);
     double *leak_n = (double *)calloc((size_t)ndir, sizeof(double));
     int64_t *nfix_n = (int64_t *)calloc((size_t)ndir, sizeof(int64_t));
     memset(phi, 0, sizeof(double) * cells * nm);
     if (nthreads < 1) nthreads = 1;
+    const int64_t cblock = 2048;                                    /* cells handled by one thread at a time in the moment sums */
+    int64_t nblocks = ((int64_t)cells + cblock - 1) / cblock;
     for (int n0 = 0; n0 < ndir; n0 += chunk) {
+        int nb = n0 + chunk <= ndir ? chunk : ndir - n0;
 #pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads)
-        for (int m = 0; m < chunk; ++m) {
+        for (int m = 0; m < nb; ++m) {
             int n = n0 + m;
             double *qn = qn_buf + cells * m, *psi = psi_buf + cells * m;
             for (size_t c = 0; c < cells; ++c) {
@@ -210,13 +218,16 @@ void orc_sweep(int nx, int ny, int nz, double dx, double dy, double dz,
             if (psi_all) memcpy(psi_all + cells * n, psi, sizeof(double) * cells);
         }
 #pragma omp parallel for schedule(static) num_threads(nthreads)
-        for (int lm = 0; lm < nm; ++lm)
-            for (int m = 0; m < chunk; ++m) {                      /* Eq. (3): fixed direction order */
-                double d = Dtab[(size_t)lm * ndir + n0 + m];
-                const double *psi = psi_buf + cells * m;
-                double *p = phi + (size_t)lm * cells;
-                for (size_t c = 0; c < cells; ++c) p[c] += d * psi[c];
-            }
+        for (int64_t blk = 0; blk < nblocks; ++blk) {                /* independent cells: any split gives the same sums */
+            size_t c0 = (size_t)(blk * cblock), c1 = c0 + (size_t)cblock < cells ? c0 + (size_t)cblock : cells;
+            for (int lm = 0; lm < nm; ++lm)
+                for (int m = 0; m < nb; ++m) {                      /* Eq. (3): fixed direction order */
+                    double d = Dtab[(size_t)lm * ndir + n0 + m];
+                    const double *psi = psi_buf + cells * m;
+                    double *p = phi + (size_t)lm * cells;
+                    for (size_t c = c0; c < c1; ++c) p[c] += d * psi[c];
+                }
+        }
     }
     double leak = 0.0;
     int64_t nf = 0;

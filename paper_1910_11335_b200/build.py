@@ -7,8 +7,10 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdoctors_b200.so")
 SOURCES = ["api.cu", "host_tables.cpp"]
-HEADERS = ["device_common.cuh", "kernels.cuh", "sweep_brick.cuh", "host_tables.h",
-           os.path.join("..", "..", "include", "doctors_b200.h")]
+def _headers():
+    """Every header the sources include: all of csrc/ plus the public header (a stale .so would be what the tests load)."""
+    here = sorted(f for f in os.listdir(CSRC) if f.endswith((".cuh", ".h")))
+    return here + [os.path.join("..", "..", "include", "doctors_b200.h")]
 
 
 def _nvcc():
@@ -22,7 +24,7 @@ def needs_build():
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(os.path.join(CSRC, f)) > t for f in SOURCES + HEADERS)
+    return any(os.path.getmtime(os.path.join(CSRC, f)) > t for f in SOURCES + _headers())
 
 
 def build(force=False, verbose=False):

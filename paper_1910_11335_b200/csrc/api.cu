@@ -16,7 +16,6 @@
 #include "host_tables.h"
 #include "kernels.cuh"
 #include "sweep_brick.cuh"
-#include "sweep_row.cuh"
 
 using namespace doctors;
 
@@ -40,9 +39,6 @@ struct Plan {
     int nprob = 0, chunk = 0, nchunks = 0, nsrc = 0, nvol = 0;
     int G = 0, L = 0, NM = 0, ndir = 0, M = 0;
     int mode = 0, sweep_mode = 0, deterministic = 0;
-    bool row = false;               // sweep_mode 2 accepted: the row-pipelined kernel (same workspace and set-up as mode 0)
-    int row_cfg = 0;                // 0: one CTA per SM, 3 stages (A); 1: two CTAs per SM, 2 stages (B)
-    size_t row_smem = 0;
     int B[3] = {0, 0, 0}, gb[3] = {0, 0, 0};
     int W = 1;                      // sweep warps per CTA
     long long nbricks = 0, ntasks = 0;
@@ -150,20 +146,6 @@ Plan make_plan(const doctors_problem* p, const doctors_solve_opts* o, int chunk)
     P.tm_inner = P.NCb / P.tm_rows;
     P.ntasks = P.nbricks * 8 * P.chunk;
     P.MT = (o && o->projection == 2) ? projection_mtiles(P.NM, P.M, P.NCb) : 0;
-    if (P.sweep_mode == 2) {
-        // row-pipelined kernel where it applies (sweep_row.cuh), else the brick kernel; everything around the launch is mode 0
-        const int skew = P.B[1] + P.B[2] - 2, rest = p->nx % P.B[0];
-        const bool shape_ok = P.M <= kMaxSweepWarps && (size_t(P.M) * P.B[0] * P.B[2]) % 2 == 0 && (size_t(P.M) * P.B[0] * P.B[1]) % 2 == 0 &&
-                              P.B[0] >= skew && (rest == 0 || rest >= skew) && P.chunk <= 255;
-        const size_t smemA = row_smem_layout(P.NM, P.B[0], P.B[1], P.B[2], P.M, 3).total;
-        const size_t smemB = row_smem_layout(P.NM, P.B[0], P.B[1], P.B[2], P.M, 2).total;
-        // A (one CTA per SM, 3 stages) where it fits, else B (two CTAs per SM, 2 stages); measured equal on config 4
-        const bool fitB = smemB <= 113 * 1024, fitA = smemA <= 227 * 1024;
-        if (shape_ok && fitA) { P.row = true; P.row_cfg = 0; P.row_smem = smemA; }
-        else if (shape_ok && fitB) { P.row = true; P.row_cfg = 1; P.row_smem = smemB; }
-        P.sweep_mode = 0;
-        if (P.row) P.MT = 0;
-    }
     P.smem = brick_smem_layout(P.NM, P.B[0], P.B[1], P.B[2], P.M, P.MT).total;
     { int dpw = (P.M + kMaxSweepWarps - 1) / kMaxSweepWarps; P.W = (P.M + dpw - 1) / dpw; }
 
@@ -633,21 +615,6 @@ cudaError_t launch_brick(const SweepLaunch& S, cudaStream_t st)
 }
 
 template <int NM, bool FIX, int MT>
-cudaError_t launch_row(const SweepLaunch& S, const RowParams& rp, int cfg, int num_sms, size_t smem, cudaStream_t st)
-{
-    if (cfg == 1) k_sweep_row<NM, FIX, 2, 4, 2, 2><<<2 * num_sms, row_threads<2, 4>(), smem, st>>>(S.tmQ, S.tmPhi, rp);
-    else k_sweep_row<NM, FIX, 3, 5, 4, 1><<<num_sms, row_threads<3, 5>(), smem, st>>>(S.tmQ, S.tmPhi, rp);
-    return cudaGetLastError();
-}
-
-template <int NM, bool FIX, int MT>
-cudaError_t prep_row(int cfg, size_t smem)
-{
-    if (cfg == 1) return cudaFuncSetAttribute(k_sweep_row<NM, FIX, 2, 4, 2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
-    return cudaFuncSetAttribute(k_sweep_row<NM, FIX, 3, 5, 4, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
-}
-
-template <int NM, bool FIX, int MT>
 cudaError_t prep_brick(size_t smem, int threads, int* max_ctas)
 {
     cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<NM, FIX, MT>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
@@ -749,7 +716,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
     const bool adaptive_window = o.check_window <= 0;   // first host read where the previous group stopped, then every sweep
     if (o.check_window <= 0) o.check_window = 12;
     if (o.closure != 0 && o.closure != 1) return fail(p, DOCTORS_INVALID_ARG, "closure must be 0 or 1");
-    if (o.sweep_mode < 0 || o.sweep_mode > 2) return fail(p, DOCTORS_INVALID_ARG, "sweep_mode must be 0, 1 or 2");
+    if (o.sweep_mode < 0 || o.sweep_mode > 1) return fail(p, DOCTORS_INVALID_ARG, "sweep_mode must be 0 or 1");
     if (o.brick[0] > 0 && (o.brick[0] % 4 != 0 || o.brick[0] > 64 || o.brick[1] <= 0 || o.brick[2] <= 0 || o.brick[1] * o.brick[2] > 32))
         return fail(p, DOCTORS_INVALID_ARG, "brick: brick[0] a multiple of 4 (<= 64), brick[1] * brick[2] <= 32 (the lanes of a warp)");
     if (!p->ws) return fail(p, DOCTORS_ALLOC, "no workspace set");
@@ -776,13 +743,12 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
     md.x0 = 0.5 * p->dx - 0.5 * nx * p->dx; md.y0 = 0.5 * p->dy - 0.5 * ny * p->dy; md.z0 = 0.5 * p->dz - 0.5 * nz * p->dz;
 
     // ---- upload inputs and tables (brick-major order; padding cells: material 0, density 0) ----
-    // x-runs of one brick row are contiguous in both orders
     auto to_bricks = [&](const auto* dense, auto* bricked) {
         for (int k = 0; k < nz; ++k)
-            for (int j = 0; j < ny; ++j)
-                for (int i0 = 0; i0 < nx; i0 += P.B[0])
-                    std::memcpy(bricked + cell_index(md, i0, j, k), dense + (size_t)nx * (j + (size_t)ny * k) + i0,
-                                sizeof(*dense) * size_t(std::min(P.B[0], nx - i0)));
+            for (int j = 0; j < ny; ++j) {
+                const auto* row = dense + (size_t)nx * (j + (size_t)ny * k);
+                for (int i = 0; i < nx; ++i) bricked[cell_index(md, i, j, k)] = row[i];
+            }
     };
     {
         std::vector<uint8_t> hm(cp, 0);
@@ -849,7 +815,6 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
     std::vector<int> oct_begin(9, 0);
     std::vector<std::vector<int32_t>> sched_off(8);
     SweepLaunch SL;
-    RowParams rowp;
     int ctas_per_sm = 0;
     if (P.sweep_mode == 0) {
         // level 2 (cells of a brick) needs no table: lane (j',k') at step s updates i' = s - j' - k' (Eq. 8)
@@ -862,30 +827,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
             int bi = b % P.gb[0], bj = (b / P.gb[0]) % P.gb[1], bk = b / (P.gb[0] * P.gb[1]);
             tasks.push_back(make_uint2(uint32_t(q) | uint32_t(oc) << 8, uint32_t(bi) | uint32_t(bj) << 10 | uint32_t(bk) << 20));
         };
-        if (P.row) {
-            // row tasks (problem, octant, bj, bk) in sub-sweep order of the (bj, bk) grid (Eq. 8 in two dimensions)
-            std::vector<std::vector<int32_t>> roff(8), rcell(8);
-            for (int oc = 0; oc < 8; ++oc) subsweep_schedule(1, P.gb[1], P.gb[2], oc, roff[oc], rcell[oc]);
-            const int rplanes = P.gb[1] + P.gb[2] - 1;
-            auto pushr = [&](int q, int oc, int r) {
-                tasks.push_back(make_uint2(uint32_t(q) | uint32_t(oc) << 8, uint32_t(r % P.gb[1]) | uint32_t(r / P.gb[1]) << 10));
-            };
-            if (!P.deterministic) {
-                for (int S = 0; S < rplanes; ++S)
-                    for (int q = 0; q < P.chunk; ++q)
-                        for (int oc = 0; oc < 8; ++oc)
-                            for (int t = roff[oc][S]; t < roff[oc][S + 1]; ++t) pushr(q, oc, rcell[oc][t]);
-                oct_begin[0] = 0; oct_begin[1] = int(tasks.size());
-            } else {
-                for (int oc = 0; oc < 8; ++oc) {
-                    oct_begin[oc] = int(tasks.size());
-                    for (int S = 0; S < rplanes; ++S)
-                        for (int q = 0; q < P.chunk; ++q)
-                            for (int t = roff[oc][S]; t < roff[oc][S + 1]; ++t) pushr(q, oc, rcell[oc][t]);
-                }
-                oct_begin[8] = int(tasks.size());
-            }
-        } else if (!P.deterministic) {
+        if (!P.deterministic) {
             // all problems and octants interleaved, brick sub-sweep S outermost
             for (int S = 0; S < gplanes; ++S)
                 for (int q = 0; q < P.chunk; ++q)
@@ -928,22 +870,6 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         ctas_per_sm = o.ctas_per_sm > 0 ? std::min(o.ctas_per_sm, max_ctas) : max_ctas;
         SL.grid = p->num_sms * ctas_per_sm;
         SL.smem = P.smem;
-        if (P.row) {
-            DISPATCH_NM_FIX(NM, o.closure == 1, 0, e = (prep_row<NM, FIX, MT>(P.row_cfg, P.row_smem)));
-            if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "row sweep kernel setup failed: %s (smem %zu)", cudaGetErrorString(e), P.row_smem);
-            ctas_per_sm = P.row_cfg == 1 ? 2 : 1;
-            RowParams& r = rowp;
-            std::memset(&r, 0, sizeof r);
-            r.nx = nx; r.ny = ny; r.nz = nz; r.BX = P.B[0]; r.BY = P.B[1]; r.BZ = P.B[2];
-            r.gbx = P.gb[0]; r.gby = P.gb[1]; r.gbz = P.gb[2]; r.M = M; r.nprob = P.chunk; r.NCb = P.NCb; r.cells_p = P.cells_p;
-            r.tm_rows = P.tm_rows; r.sigt = at<double>(p, P.o_sigt); r.octtab = at<unsigned char>(p, P.o_octtab);
-            r.Gs = G; r.tasks = at<uint2>(p, P.o_tasks); r.ctl = at<Control>(p, P.o_ctl); r.flags = at<unsigned>(p, P.o_flags);
-            r.faceY = at<double>(p, P.o_fy); r.faceZ = at<double>(p, P.o_fz);
-            r.state = at<ProbState>(p, P.o_state); r.leak = at<double>(p, P.o_leak);
-#ifdef DOCTORS_TIMING
-            { static long long* dt = nullptr; if (!dt) { cudaMalloc(&dt, 32 * 8); } cudaMemset(dt, 0, 32 * 8); r.dbg_time = dt; }
-#endif
-        }
         BrickParams& bp = SL.bp;
         bp.nx = nx; bp.ny = ny; bp.nz = nz;
         bp.BX = P.B[0]; bp.BY = P.B[1]; bp.BZ = P.B[2];
@@ -957,11 +883,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         bp.flags = at<unsigned>(p, P.o_flags);
         bp.faceX = at<double>(p, P.o_fx); bp.faceY = at<double>(p, P.o_fy); bp.faceZ = at<double>(p, P.o_fz);
         bp.dbg_plane = nullptr;
-        bp.dbg_time = nullptr;
         bp.bulk_faces = (P.face_x_n % 2 == 0 && P.face_y_n % 2 == 0 && P.face_z_n % 2 == 0) ? 1 : 0;
-#ifdef DOCTORS_TIMING
-        { static long long* dt = nullptr; if (!dt) { cudaMalloc(&dt, 16 * 8); } cudaMemset(dt, 0, 16 * 8); bp.dbg_time = dt; }
-#endif
         bp.state = at<ProbState>(p, P.o_state);
         bp.leak = at<double>(p, P.o_leak);
     } else {
@@ -1064,11 +986,6 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
                             // problems done (k_group_begin), so their tasks are skipped
                             SL.bp.ntasks = oct_begin[l + 1] - oct_begin[l];
                             cudaError_t e;
-                            if (P.row) {
-                                rowp.g = g; rowp.epoch = SL.bp.epoch; rowp.counter_slot = l;
-                                rowp.task_begin = SL.bp.task_begin; rowp.ntasks = SL.bp.ntasks;
-                                DISPATCH_NM_FIX(NM, o.closure == 1, 0, e = (launch_row<NM, FIX, MT>(SL, rowp, P.row_cfg, p->num_sms, P.row_smem, st)));
-                            } else
                             DISPATCH_NM_FIX(NM, o.closure == 1, P.MT, e = (launch_brick<NM, FIX, MT>(SL, st)));
                             if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "sweep launch failed: %s", cudaGetErrorString(e));
                             ++sweep_launches; ++kernel_launches;
@@ -1118,23 +1035,6 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
     CK(cudaStreamSynchronize(st));
     CK(cudaGetLastError());
 
-#ifdef DOCTORS_TIMING
-    if (P.row && rowp.dbg_time) {
-        long long h[32];
-        cudaMemcpy(h, rowp.dbg_time, sizeof h, cudaMemcpyDeviceToHost);
-        const char* nm[20] = {"loader total", "loader wait phase 2", "loader wait reduce read", "-", "z poller total", "poller wait face slot", "poller flag spin", "-",
-                              "publisher total", "publisher wait wave", "publisher wait store", "-", "proj total", "proj wait tile", "proj wait wave", "-",
-                              "wave total", "wave wait phase 0", "wave wait faces", "-"};
-        for (int i = 0; i < 20; ++i) if (nm[i][0] != '-') fprintf(stderr, "  [row timing] %-26s %.3e cycles (%5.1f %% of its role)\n", nm[i], double(h[i]), 100.0 * h[i] / double(h[i / 4 * 4]));
-    }
-    if (!P.row && P.sweep_mode == 0 && SL.bp.dbg_time) {
-        long long h[16];
-        cudaMemcpy(h, SL.bp.dbg_time, sizeof h, cudaMemcpyDeviceToHost);
-        const char* nm[12] = {"fetch", "dep: tables+sync", "face-load", "tma-wait", "phase0", "wavefront", "face-store+release", "phase2", "tail", "dep: reduce-read wait + TMA issue", "dep: flag poll", "-"};
-        double tot = 0; for (int i = 0; i < 12; ++i) tot += double(h[i]);
-        for (int i = 0; i < 12; ++i) fprintf(stderr, "  [timing] %-20s %6.2f %%  %.3e cycles\n", nm[i], 100.0 * h[i] / tot, double(h[i]));
-    }
-#endif
     // ---- results ----
     std::vector<GroupResult> res(size_t(P.nprob) * G);
     CK(cudaMemcpy(res.data(), at<GroupResult>(p, P.o_results), res.size() * sizeof(GroupResult), cudaMemcpyDeviceToHost));
@@ -1164,7 +1064,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         info->brick[0] = P.B[0]; info->brick[1] = P.B[1]; info->brick[2] = P.B[2];
         info->ctas_per_sm = ctas_per_sm;
         info->projection_mtiles = P.sweep_mode == 0 ? P.MT : 0;
-        info->sweep_kernel = o.sweep_mode == 1 ? 1 : (P.row ? 2 : 0);
+        info->sweep_kernel = o.sweep_mode == 1 ? 1 : 0;
     }
     for (auto e : sweep_ev) cudaEventDestroy(e);
     for (auto e : fixed_ev) cudaEventDestroy(e);
@@ -1250,15 +1150,19 @@ extern "C" int doctors_debug_device_brick_steps(doctors_problem* p, int bx, int 
     bp.tasks = S.task; bp.ctl = S.ctl; bp.flags = S.flags;
     bp.faceX = S.face; bp.faceY = S.face + size_t(by) * bz; bp.faceZ = bp.faceY + size_t(bx) * bz;
     bp.state = S.st; bp.leak = S.leak;
-    bp.dbg_time = nullptr; bp.dbg_plane = S.planes;
+    bp.dbg_plane = S.planes;
     cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<1, false, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
     if (e == cudaSuccess) {
         k_sweep_brick<1, false, 0, true><<<1, 32, smem, p->stream>>>(SL.tmQ, SL.tmPhi, bp);
         e = cudaGetLastError();
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
-    if (e == cudaSuccess) e = cudaMemcpy(step_of_cell, S.planes, size_t(NC) * 4, cudaMemcpyDeviceToHost);
+    std::vector<int32_t> stored(size_t(NC), -1);
+    if (e == cudaSuccess) e = cudaMemcpy(stored.data(), S.planes, size_t(NC) * 4, cudaMemcpyDeviceToHost);
     cudaFree(base);
+    for (int lk = 0; lk < bz; ++lk)                             // storage order inside a brick (y fastest) -> documented order
+        for (int lj = 0; lj < by; ++lj)
+            for (int li = 0; li < bx; ++li) step_of_cell[li + bx * (lj + by * lk)] = stored[size_t(lj + by * (li + bx * lk))];
     if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "debug brick launch failed: %s", cudaGetErrorString(e));
     return DOCTORS_OK;
 }

@@ -11,11 +11,17 @@ constexpr int kMaxMoments = 16;       // P3
 constexpr int kMaxSweepWarps = 10;   // sweep CTA = one warp per direction of the octant (looped if M > 10)
 
 // Device storage order of every per-cell array is BRICK-MAJOR: cell (i,j,k) lives at
-//   cp = brick * NCb + li + BX*(lj + BY*lk),  brick = bi + gbx*(bj + gby*bk),  (bi,li) = divmod(i, BX) ...
+//   cp = brick * NCb + lj + BY*(li + BX*lk),  brick = bi + gbx*(bj + gby*bk),  (bi,li) = divmod(i, BX) ...
 // so that the tile a sweep task loads (one brick, one moment) is ONE contiguous run of NCb*4 bytes
 // instead of BY*BZ rows of BX*4 bytes (64-byte rows made the TMA unit fetch whole 128-byte lines: 2x
-// read amplification on Q, measured in round 1).  Bricks at the mesh edge are padded with inert cells
-// (density 0, all fields 0).  The ray tracer alone also reads dense x-fastest copies of material / density.
+// read amplification on Q, measured in round 1).  INSIDE a brick y runs fastest, then x, then z: the
+// wavefront's 32 lanes (j',k') touch, at step s, the cells i' = s - j' - k', i.e. local indices
+// 8 s - 7 j' + 8 (BX - 1) k' for an 8 x 4 cross section — 32 different banks for every even BX (and 16
+// different 8-byte bank pairs per half warp for sigma_t).  With x fastest the same lanes sat at
+// (BX - 1) j' + (BX BY - 1) k', which collides for every even BX: 21 % of the shared-memory wavefronts of the
+// round-1 kernel were bank-conflict replays (profiles/r02_sweep_ncu.md).
+// Bricks at the mesh edge are padded with inert cells (density 0, all fields 0).  The ray tracer alone also
+// reads dense x-fastest copies of material / density.
 struct MeshDev {
     int nx, ny, nz;
     int BX, BY, BZ;         // brick extents
@@ -29,13 +35,13 @@ __host__ __device__ __forceinline__ long long cell_index(const MeshDev& m, int i
 {
     const int bi = i / m.BX, bj = j / m.BY, bk = k / m.BZ;
     const int li = i - bi * m.BX, lj = j - bj * m.BY, lk = k - bk * m.BZ;
-    return (long long)(bi + m.gbx * (bj + m.gby * bk)) * m.NCb + li + m.BX * (lj + m.BY * lk);
+    return (long long)(bi + m.gbx * (bj + m.gby * bk)) * m.NCb + lj + m.BY * (li + m.BX * lk);
 }
 // returns false for a padding cell
 __host__ __device__ __forceinline__ bool cell_ijk(const MeshDev& m, long long cp, int& i, int& j, int& k)
 {
     const int brick = int(cp / m.NCb), local = int(cp - (long long)brick * m.NCb);
-    const int li = local % m.BX, t = local / m.BX, lj = t % m.BY, lk = t / m.BY;
+    const int lj = local % m.BY, t = local / m.BY, li = t % m.BX, lk = t / m.BX;
     const int bi = brick % m.gbx, u = brick / m.gbx, bj = u % m.gby, bk = u / m.gby;
     i = bi * m.BX + li; j = bj * m.BY + lj; k = bk * m.BZ + lk;
     return i < m.nx && j < m.ny && k < m.nz;

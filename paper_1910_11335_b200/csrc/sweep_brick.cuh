@@ -62,7 +62,6 @@ struct BrickParams {
     const ProbState* state;
     double* leak;                // [prob]
     int bulk_faces;              // 1: all three face blocks are multiples of 16 bytes -> moved by bulk async copies (TMA unit)
-    long long* dbg_time;         // -DDOCTORS_TIMING builds only: [16] cycle sums per phase (thread 0 of every CTA)
     int* dbg_plane;              // debug hook: NULL, or [BX*BY*BZ] receives the step at which each cell of a full brick is visited
 };
 
@@ -106,7 +105,10 @@ __host__ __device__ inline BrickSmem brick_smem_layout(int NM, int BX, int BY, i
 {
     BrickSmem s;
     size_t NC = size_t(BX) * BY * BZ, o = 0;
-    s.misc = o;  o = align_up(o + 128, 128);   // mbarrier, task slots, reduction scratch; also the pad idle lanes may read
+    s.misc = o;  o = align_up(o + 128, 128);   // mbarrier, task slots, reduction scratch
+    // front pad: a wavefront lane that has not reached its x range yet loads from its running address, up to
+    // (BY + BZ - 2) steps of BY cells (8 bytes each for sigma_t) BEFORE its row — that must still be this CTA's memory
+    o = align_up(o + size_t(8) * BY * (BY + BZ - 2), 128);
     // one tile of max(NM, M) planes holds, in turn, Q_lm (bulk loads), psi_n (in place, per cell) and the
     // phi_lm contribution (in place again, bulk reduce-add source)
     s.q = o;     o = align_up(o + size_t(NM > M ? NM : M) * plane_pitch(int(NC), MT) * 4, 128);
@@ -117,7 +119,7 @@ __host__ __device__ inline BrickSmem brick_smem_layout(int NM, int BX, int BY, i
     s.fz = o;    o = align_up(o + size_t(M) * BX * BY * 8, 16);
     s.tab = o;   o = align_up(o + octtab_layout(NM, M, MT).total, 16);
     s.done = o;  o = align_up(o + 256, 16);      // "problem has stopped" bytes of the launch (task prob index is 8 bits)
-    o = align_up(o + 128, 16);                  // tail pad (idle lanes may read up to 10 cells past the tables' start)
+    o = align_up(o + 128 + size_t(8) * BY * (BY + BZ - 2), 16);   // tail pad: lanes past their x range (sx < 0: before it) overshoot by the same amount
     s.total = o;
     return s;
 }
@@ -326,12 +328,6 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
     const int faceXn = M * BY * BZ, faceYn = M * BX * BZ, faceZn = M * BX * BY;
     const int nbricks = P.gbx * P.gby * P.gbz;
     int last_oct = -1;
-#ifdef DOCTORS_TIMING
-    long long tacc[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, tprev = clock64();
-#define TICK(i) do { if (tid == 0) { long long t_ = clock64(); tacc[i] += t_ - tprev; tprev = t_; } } while (0)
-#else
-#define TICK(i) do { } while (0)
-#endif
 
     // Roles inside the CTA (all of them also sweep):
     //   tile warp   lanes 0..NM-1 own one moment plane each: bulk load of Q_lm at the start of a task, bulk reduce-add of
@@ -378,7 +374,6 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         const int prob_done = sDoneP[td.x & 0xff];
         if (tid == pfThread) fetch_task(slot ^ 1);
         slot ^= 1;
-        TICK(0);
         if (prob_done) continue;                                 // this problem has stopped (a6)
         const int prob = td.x & 0xff, oct = (td.x >> 8) & 7;
         const int bi = td.y & 0x3ff, bj = (td.y >> 10) & 0x3ff, bk = (td.y >> 20) & 0x3ff;
@@ -421,7 +416,6 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
             if (tab && lane == 17) bulk_load(smem_u32(smem + L.tab), P.octtab + (size_t)oct * T.total, uint32_t(T.total), bar);
         }
         last_oct = oct;
-        TICK(9);
         // wait for the upwind bricks of this (problem, octant): one warp-0 lane per upwind flag
         if (P.bulk_faces) {
             if (warp == 0 && lane < 3) {
@@ -450,8 +444,6 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
             }
             __syncthreads();                                     // flags seen by warp 0 -> everyone may read faces
         }
-        TICK(10);
-        TICK(1);
 
         // inflow faces: upwind brick's outflow, or vacuum.  sFx, sFy, sFz are contiguous.
         const int nxy = faceXn + faceYn, nall = nxy + faceZn;
@@ -477,10 +469,8 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
                 sFx[e] = u ? __ldcg(src) : 0.0;
             }
         }
-        TICK(2);
         mbar_wait(bar, parity);
         parity ^= 1u;
-        TICK(3);
 
         // ---- phase 0: q_n = sum_lm Mtab[n][lm] Q_lm for every cell of the brick (a5) ----
         if constexpr (MT >= 1) {
@@ -530,7 +520,6 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
             }
         }
         __syncthreads();
-        TICK(4);
 
         // ---- wavefront (a3 level 2, a4): warp = direction, lanes = (j',k'), step s -> plane i'+j'+k' = s ----
         const bool edge_x = !dnx, edge_y = !dny, edge_z = !dnz;  // outflow faces on the mesh boundary
@@ -540,17 +529,17 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         const int nsteps = ex + ey + ez - 2;
         const bool last_y = jp == ey - 1, last_z = kp == ez - 1;
         const int li0 = (sx > 0 ? 0 : ex - 1) - sx * (jp + kp);   // li at step 0 (i' = -(j'+k')), advanced by sx per step
-        const uint32_t row = uint32_t(BX * (lj + BY * lk_) + li0);
+        const uint32_t row = uint32_t(lj + BY * (li0 + BX * lk_));    // local index: y fastest, then x, then z (device_common.cuh)
         const bool first_y = jp == 0, first_z = kp == 0;
         // Idle lanes (before / after their x range) load from wherever their running address points — always
         // inside this CTA's shared memory, which starts with a 128-byte pad and ends with the tables — and
         // compute on that garbage; only stores and the x-face register are predicated.  Clipped lanes
         // (beyond ey / ez) stay parked on the tile's first cell.
-        int d4 = lane_ok ? 4 * sx : 0, d8 = 2 * d4;
+        int d4 = lane_ok ? 4 * sx * BY : 0, d8 = 2 * d4, d8f = lane_ok ? 8 * sx : 0;   // one cell along x: tile (fp32), sigma_t (fp64), face rows (fp64)
         int shy = BY, ly = last_y ? 1 : 0, lz = last_z ? 1 : 0;
         // loop invariants pinned in registers: otherwise the compiler re-derives them every step (constant-bank reads,
         // ey - 1 / ez - 1 on the uniform datapath, 2 * d4)
-        asm volatile("" : "+r"(d4), "+r"(d8), "+r"(shy), "+r"(ly), "+r"(lz));
+        asm volatile("" : "+r"(d4), "+r"(d8), "+r"(d8f), "+r"(shy), "+r"(ly), "+r"(lz));
         for (int n = warp; n < M; n += P.W) {
             const double cx = sDir[4 * n], cy = sDir[4 * n + 1], cz = sDir[4 * n + 2], cs = sDir[4 * n + 3];
             double* fxp = sFx + n * (BY * BZ) + lj + BY * lk_;
@@ -576,13 +565,12 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
                 sts_f64_if(act && ly, py, oy);
                 sts_f64_if(act && lz, pz, oz);
                 if (act) ax = ox;
-                if (DBG && act) P.dbg_plane[(pq - smem_u32(sPsi)) / 4u - uint32_t(n * NCP)] = nsteps - s;
-                ++ip; pq += d4; ps += d8; py += d8; pz += d8;
+                if (DBG && act) P.dbg_plane[(pq - smem_u32(sPsi)) / 4u - uint32_t(n * NCP)] = nsteps - s;   // indexed by the storage order (y fastest)
+                ++ip; pq += d4; ps += d8; py += d8f; pz += d8f;
             }
             if (lane_ok) *fxp = ax;
         }
         __syncthreads();
-        TICK(5);
 
         // leakage through the mesh boundary (balance report): sum of w |Omega_d| A_d psi_out over boundary faces
         if (edge_x | edge_y | edge_z) {
@@ -621,7 +609,6 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
             __syncthreads();
             if (tid == nthr - 1) st_release_u32(flag_base + brick, P.epoch);   // cumulative: covers the CTA's face stores (ordered by the barrier)
         }
-        TICK(6);
 
         // ---- phase 2: phi_lm += sum_n Dtab[n][lm] psi_n (Eq. 3, a5), tile -> sQ, bulk reduce-adds ----
         if constexpr (MT >= 1) {
@@ -663,7 +650,6 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         }
         fence_proxy_async_smem();
         __syncthreads();
-        TICK(7);
         if (warp == tileWarp) {
             if constexpr (MT == 0) {
                 if (lane == 0) {
@@ -687,13 +673,6 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         }
     }
     if (warp == tileWarp) bulk_wait0();
-#ifdef DOCTORS_TIMING
-    if (tid == 0 && P.dbg_time) {
-        tacc[8] = clock64() - tprev;
-        for (int i = 0; i < 12; ++i) atomicAdd(reinterpret_cast<unsigned long long*>(P.dbg_time) + i, (unsigned long long)tacc[i]);
-    }
-#endif
-#undef TICK
 }
 
 }  // namespace doctors

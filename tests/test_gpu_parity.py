@@ -133,33 +133,6 @@ def test_projection_paths_p3(pkg, orc, sn, mtiles, brick):
     assert np.abs(got[2] - got[1]).max() / scale < 2e-5
 
 
-@pytest.mark.parametrize("closure,det", [(0, 0), (1, 0), (1, 1)])
-def test_row_pipelined_kernel(pkg, orc, closure, det):
-    """sweep_mode 2: one CTA per SM sweeps x-rows of bricks through a three-stage pipeline (sweep_row.cuh).
-    60x19x10 mesh with 12x8x4 bricks: rows of 5 bricks, clipped bricks in y and z, scalar flux and particle balance.
-    64x9x6: the last brick of a row (4 cells) is shorter than the in-brick skew, so the library falls back to the brick kernel."""
-    wl = tiny_p3_case(nx=60, ny=19, nz=10, G=2, sn=8, L=3, seed=9)
-    ref = orc.solve(wl, closure=closure)
-    p, info = run_gpu(wl, closure=closure, fixed_iters=ref["iters"], sweep_mode=2, brick=(12, 8, 4), deterministic=det)
-    assert info["sweep_kernel"] == 2
-    shape = (wl.nz, wl.ny, wl.nx)
-    for g in range(wl.G):
-        e, _ = masked_rel_err(p.get_flux_moments(0, g, 0)[0], ref["phi"][0, g, 0].reshape(shape))
-        assert e < TOL, (g, e)
-        src, col, leak = info["balance"][0, g]
-        assert abs(src - col - leak) < 2e-5 * src               # per-sweep particle balance (leakage summed by the wavefront warps)
-        np.testing.assert_allclose(info["balance"][0, g], ref["balance"][0, g], rtol=2e-5)
-    p.close()
-    # where the row kernel does not apply the brick kernel runs: last brick of the row shorter than the in-brick skew
-    wl2 = tiny_p3_case(nx=64, ny=9, nz=6, G=1, sn=8, L=3, seed=9)
-    ref2 = orc.solve(wl2, closure=closure)
-    p, info = run_gpu(wl2, closure=closure, fixed_iters=ref2["iters"], sweep_mode=2, brick=(12, 8, 4))
-    assert info["sweep_kernel"] == 0
-    e, _ = masked_rel_err(p.get_flux_moments(0, 0, 0)[0], ref2["phi"][0, 0, 0].reshape((wl2.nz, wl2.ny, wl2.nx)))
-    assert e < TOL
-    p.close()
-
-
 def test_degenerate_meshes(pkg, orc):
     for dims in [(1, 1, 1), (1, 7, 3), (5, 1, 1), (17, 2, 1)]:
         wl = tiny_p3_case(nx=dims[0], ny=dims[1], nz=dims[2], G=2, sn=4, L=1, seed=3)
