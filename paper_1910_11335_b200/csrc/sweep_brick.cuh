@@ -323,7 +323,6 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
 
     const uint32_t barF = bar + 32;                                  // faces (bulk copies) complete here
     if (tid == 0) { mbar_init(bar, 1); mbar_init(barF, P.bulk_faces ? 3 : 1); fence_mbar_init(); }
-    __syncthreads();
     uint32_t parity = 0;
     const int faceXn = M * BY * BZ, faceYn = M * BX * BZ, faceZn = M * BX * BY;
     const int nbricks = P.gbx * P.gby * P.gbz;
@@ -353,28 +352,18 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         sDesc[sl] = d; sTask[sl] = id;
     };
     if (tid == 0) fetch_task(0);
+    __syncthreads();                                             // mbarriers, first task, stop flags
     int slot = 0;
-    bool publish = false;                                        // publishing warp: a brick waits to be published
-    unsigned* pub_flag = nullptr;
+    // ONE block barrier ends a task (after phase 2): behind it nobody reads the tile, the tables, the faces or the task
+    // slot of that task any more, so the next task starts without a barrier of its own.
     while (true) {
-        if (publish && lane == 31) bulk_wait_read0();            // the face blocks have been read out of sFx..sFz
-        bar_sync1(nthr);
-        if (publish) {
-            // the other 31 lanes run ahead to the tile wait of the next task; this one joins them there
-            if (lane == 31) {
-                bulk_wait0();                                    // the face blocks are in global memory
-                fence_proxy_async_global();
-                st_release_u32(pub_flag, P.epoch);
-            }
-            publish = false;
-        }
         const int t = sTask[slot];
         if (t >= P.ntasks) break;
         const uint2 td = sDesc[slot];
         const int prob_done = sDoneP[td.x & 0xff];
         if (tid == pfThread) fetch_task(slot ^ 1);
         slot ^= 1;
-        if (prob_done) continue;                                 // this problem has stopped (a6)
+        if (prob_done) { __syncthreads(); continue; }            // this problem has stopped (a6); the barrier orders the task slots
         const int prob = td.x & 0xff, oct = (td.x >> 8) & 7;
         const int bi = td.y & 0x3ff, bj = (td.y >> 10) & 0x3ff, bk = (td.y >> 20) & 0x3ff;
 
@@ -570,7 +559,15 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
             }
             if (lane_ok) *fxp = ax;
         }
+        if (P.bulk_faces) fence_proxy_async_smem();              // lanes' face writes -> visible to the async proxy
         __syncthreads();
+        // ---- outflow faces to the downwind bricks: bulk async stores issued by the publisher (last lane of the last warp) ----
+        if (P.bulk_faces && warp == pubWarp && lane == 31) {
+            if (dnx) bulk_store(gFx, smem_u32(sFx), uint32_t(8 * faceXn));
+            if (dny) bulk_store(gFy, smem_u32(sFy), uint32_t(8 * faceYn));
+            if (dnz) bulk_store(gFz, smem_u32(sFz), uint32_t(8 * faceZn));
+            bulk_commit();
+        }
 
         // leakage through the mesh boundary (balance report): sum of w |Omega_d| A_d psi_out over boundary faces
         if (edge_x | edge_y | edge_z) {
@@ -592,17 +589,7 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
             if (lane == 0) sRed[warp] = lk;
         }
 
-        // ---- outflow faces to the downwind bricks, then publish the brick ----
-        if (P.bulk_faces) {
-            fence_proxy_async_smem();                            // lanes' face writes -> visible to the async proxy
-            __syncthreads();
-            if (warp == pubWarp && lane == 31) {
-                if (dnx) bulk_store(gFx, smem_u32(sFx), uint32_t(8 * faceXn));
-                if (dny) bulk_store(gFy, smem_u32(sFy), uint32_t(8 * faceYn));
-                if (dnz) bulk_store(gFz, smem_u32(sFz), uint32_t(8 * faceZn));
-                bulk_commit();
-            }
-        } else {
+        if (!P.bulk_faces) {                                     // odd-sized face blocks: plain stores, flag after a barrier
             if (dnx) for (int e = tid; e < faceXn; e += nthr) __stcg(gFx + e, sFx[e]);
             if (dny) for (int e = tid; e < faceYn; e += nthr) __stcg(gFy + e, sFy[e]);
             if (dnz) for (int e = tid; e < faceZn; e += nthr) __stcg(gFz + e, sFz[e]);
@@ -648,8 +635,10 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
                 }
             }
         }
+        const bool publisher = P.bulk_faces && warp == pubWarp && lane == 31;
+        if (publisher) bulk_wait_read0();                        // the face blocks have been read out of sFx..sFz (issued before phase 2)
         fence_proxy_async_smem();
-        __syncthreads();
+        __syncthreads();                                         // end of the task
         if (warp == tileWarp) {
             if constexpr (MT == 0) {
                 if (lane == 0) {
@@ -667,9 +656,10 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
             for (int w = 0; w < P.W; ++w) s += sRed[w];
             atomicAdd(P.leak + prob, (double)s);
         }
-        if (P.bulk_faces && warp == pubWarp) {                   // published at the loop top, after arriving at the barrier
-            publish = true;
-            pub_flag = flag_base + brick;
+        if (publisher) {                                         // the other lanes of its warp are already on the next task
+            bulk_wait0();                                        // the face blocks are in global memory
+            fence_proxy_async_global();
+            st_release_u32(flag_base + brick, P.epoch);
         }
     }
     if (warp == tileWarp) bulk_wait0();
