@@ -27,8 +27,12 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+CONFIG_LABEL = {0: "cfg0_8c_S2P0", 1: "cfg1_32c_sphere_S8P3", 2: "cfg2_64c_cyl_S8P3", 3: "cfg3_128x128x64_S16P3",
+                4: "cfg4_256x256x128_S8P3_8src"}
 METRIC = "cell_direction_group_updates_per_s"
 UNIT = "updates/s"
+TRAFFIC_CSV = "r02_sweep_traffic.csv"
+NOMINAL_HBM_GBS = 8000.0      # the ~8 TB/s BASELINE.json north_star quotes
 
 
 def rank_world():
@@ -46,9 +50,9 @@ def measured_peak():
 
 def ncu_traffic_per_problem_sweep(idx):
     """DRAM bytes (read + write) one problem's share of a sweep launch moved under `ncu --set full`, from the committed
-    summary profiles/r01_sweep_traffic.csv (columns: config, problems_in_launch, dram_read_bytes, dram_write_bytes)."""
+    summary profiles/r02_sweep_traffic.csv (columns: config, problems_in_launch, dram_read_bytes, dram_write_bytes, commit)."""
     try:
-        with open(os.path.join(ROOT, "profiles", "r01_sweep_traffic.csv")) as f:
+        with open(os.path.join(ROOT, "profiles", TRAFFIC_CSV)) as f:
             for ln in f:
                 c = ln.strip().split(",")
                 if len(c) >= 4 and c[0].strip() == str(idx):
@@ -153,7 +157,10 @@ def oracle_sample(idx):
         wl.name, sweeps, wl.n_dir)
 
 
-def time_oracle(wl, closure):
+def time_oracle(wl, closure, one_thread=True):
+    """The fp64 oracle as it stands on the host cores: sweeps timed apart from the ray trace and the fixed-source
+    assembly (oracle.solve reports the split), all cores and — BASELINE.md §2, the paper's CPU configuration
+     — one thread.  Returns the cpu_baseline object."""
     from oracle import oracle
     oracle.build()
     cores = oracle.default_threads()
@@ -161,7 +168,19 @@ def time_oracle(wl, closure):
     res = oracle.solve(wl, closure=closure, threads=cores)
     dt = time.perf_counter() - t0
     updates = int(res["iters"].sum()) * wl.cells * wl.n_dir
-    return updates, dt, cores
+    sec = {k: float(v) for k, v in res["seconds"].items()}
+    out = {"value": updates / sec["sweep"], "unit": UNIT, "cores": cores, "kind": "oracle",
+           "what": "untuned fp64 oracle (test infrastructure), sweeps only; not a tuned CPU solver",
+           "updates": updates, "seconds": dict(sec, total=dt), "value_incl_raytrace_and_source": updates / dt}
+    if one_thread and cores > 1:
+        import copy
+        w1 = copy.copy(wl)
+        w1.fixed_iters = 1                                   # one sweep per group of the same sample, on one thread
+        r1 = oracle.solve(w1, closure=closure, threads=1, raytrace_threads=cores)
+        u1 = int(r1["iters"].sum()) * wl.cells * wl.n_dir
+        out["value_1thread"] = u1 / r1["seconds"]["sweep"]
+        out["seconds_1thread_sweep"] = float(r1["seconds"]["sweep"])
+    return out
 
 
 def run_reference(args):
@@ -169,20 +188,26 @@ def run_reference(args):
     if rank != 0:
         return 0
     wl, sample = oracle_sample(args.config)
-    full = workload_for(args.config) if args.config > 1 else wl
-    times, updates, cores = [], 0, 0
+    steps = []
     for i in range(args.warmup + args.steps):
-        u, dt, cores = time_oracle(wl, args.closure)
+        c = time_oracle(wl, args.closure, one_thread=False)
         if i >= args.warmup:
-            times.append(dt); updates += u
-    total = sum(times)
-    v = updates / total
+            steps.append(c)
+    updates = sum(c["updates"] for c in steps)
+    sweep_s = sum(c["seconds"]["sweep"] for c in steps)
+    total_s = sum(c["seconds"]["total"] for c in steps)
+    v = updates / sweep_s
+    cfg = bench_config(wl, args, None)                       # the workload that RAN: the bounded sample, named as such
+    cfg["sample_of"] = CONFIG_LABEL.get(args.config, "config %d" % args.config)
+    cfg["sample"] = sample
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": 1e3 * total / max(1, args.steps), "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": bench_config(full, args, None),
-            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
-            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "warmup": args.warmup, "ms_per_step": 1e3 * total_s / max(1, args.steps), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfg,
+            "ms_per_step_split": {k: 1e3 * sum(c["seconds"][k] for c in steps) / max(1, args.steps)
+                                  for k in ("raytrace", "fixed_source", "sweep")},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": steps[-1]["cores"], "kind": "oracle", "sample": sample,
+                             "what": steps[-1]["what"]},
+            "e2e": {"value": updates / total_s, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
     return 0
@@ -261,13 +286,14 @@ def run_gpu_arm(args):
         dist.barrier()
     sampler = ClockSampler(dev) if rank == 0 else None
     ms_dev = ms_sweep = 0.0
-    updates = launches = sweep_launches = 0
+    updates = launches = sweep_launches = timed_sweeps = 0
     t0 = time.perf_counter()
     info = None
     for _ in range(args.steps):
         info = step()
         ms_dev += info["ms_total"]; ms_sweep += info["ms_sweep"]
         updates += info["updates"]; launches += info["kernel_launches"]; sweep_launches += info["sweep_launches"]
+        timed_sweeps += info["timed_sweeps"]
     torch.cuda.synchronize()
     if dist is not None:
         dist.barrier()
@@ -322,7 +348,10 @@ def run_gpu_arm(args):
         if per is not None:
             traffic = per * problem_sweeps / max(1, sweep_launches)
     roofline = {"bound": "hbm", "kernel": "k_sweep_brick", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "peak_source": peak_src, "traffic": traffic, "traffic_unit": "DRAM bytes per launch (ncu, profiles/r01_sweep_traffic.csv)",
+                "frac": achieved / peak, "peak_source": peak_src, "frac_of_nominal_8tbs": achieved / NOMINAL_HBM_GBS,
+                "traffic": traffic, "traffic_unit": "DRAM bytes per launch (one ncu --set full capture of this kernel on the config's "
+                "2-problem slice, profiles/%s, scaled to this run's problems per launch)" % TRAFFIC_CSV,
+                "timed_sweeps": int(timed_sweeps),
                 "launches": int(sweep_launches), "avg_launch_ms": ms_sweep / max(1, sweep_launches),
                 "algorithmic_bytes_per_launch": alg_bytes / max(1, sweep_launches),
                 "share_of_step": ms_sweep / ms_dev,
@@ -332,8 +361,8 @@ def run_gpu_arm(args):
     cpu = None
     if world == 1 and not args.no_cpu:
         swl, sample = oracle_sample(args.config)
-        u, dt, cores = time_oracle(swl, args.closure)
-        cpu = {"value": u / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "seconds": dt}
+        cpu = time_oracle(swl, args.closure)
+        cpu["sample"] = sample
 
     value = upd_all / (ms_all * 1e-3)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

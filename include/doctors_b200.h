@@ -121,7 +121,8 @@ typedef struct {
     int check_window;         /* tolerance mode: sweeps enqueued between host reads of the device flag; 0 = adaptive
                                * (first read one sweep before the count the previous group needed, then every sweep) */
     int projection;           /* sweep_mode 0, the two projections of Eq. (2) rhs / Eq. (3) inside the sweep kernel:
-                               * 0 automatic (= 1: the fastest measured on B200), 1 packed fp32 FMA loops,
+                               * 0 automatic: tensor cores for more than 16 directions per octant (S12, S16), else the FMA loops
+                               *   (the faster of the two as measured on B200); 1 packed fp32 FMA loops;
                                * 2 tensor cores (mma TF32, 3-product split, fp32 accumulate) when P3, <= 48 directions per
                                *   octant and a brick of a multiple of 8 cells; else the FMA loops */
 } doctors_solve_opts;
@@ -139,6 +140,10 @@ typedef struct {
     int ctas_per_sm;
     int sweep_kernel;         /* kernel that swept: 0 brick, 1 paper scheme */
     int projection_mtiles;    /* > 0: the projections ran on the tensor cores (16-direction m-tiles per octant); 0: fp32 FMA loops */
+    unsigned long long timed_sweeps;   /* sweep iterations whose CUDA-event time is in ms_sweep (= all of them) */
+    int pl_exceeds_quadrature;/* warning flag: 1 if the quadrature does not integrate Y_lm Y_l'm' exactly up to pl_order
+                               * (level-symmetric sets: exact up to P1 / P2 / P3 / P4 at S2 / S4 / S6 / S8, >= P5 at S12 / S16;
+                               * e.g. P3 with S4).  The solve runs; the scattering-source moments are then not Galerkin-consistent. */
 } doctors_solve_info;
 
 /* n_problems = n_sources (mode 0) or 1 (mode 1). */
@@ -207,6 +212,11 @@ int doctors_host_level_symmetric(int sn_order, double* omega_xyz, double* w);
 int doctors_host_schedule(int nx, int ny, int nz, int octant, int32_t* plane_offset, int32_t* cell_of);
 int doctors_host_projection_tables(int pl_order, int n_dir, const double* omega_xyz, const double* w,
                                    double* Mtab, double* Dtab);
+/* The warning doctors_solve_info.pl_exceeds_quadrature as a host function: returns 1 if the set does NOT integrate the
+ * products Y_lm Y_l'm' exactly for all l, l' <= pl_order (defect = max |sum_n w_n Y_lm (2l'+1)/(4 pi) Y_l'm' - delta| > 1e-9),
+ * 0 if it does, -1 for bad arguments; *defect (may be NULL) receives the defect.  Level-symmetric sets are exact up to
+ * P1 / P2 / P3 / P4 at S2 / S4 / S6 / S8 and beyond P3 at S12 / S16 (quadrature rule). */
+int doctors_host_pl_exceeds_quadrature(int pl_order, int n_dir, const double* omega_xyz, const double* w, double* defect);
 
 #ifdef __cplusplus
 }

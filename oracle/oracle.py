@@ -243,7 +243,8 @@ def unit_dirs_from(wl, pos):
 # --------------------------------------------------------------------------------------
 # Multigroup source iteration (PAPER.md:34 Eq. 2, :44-62 Eqs. 4-7, :149, :183)
 # --------------------------------------------------------------------------------------
-def solve(wl, closure=0, fixed_iters=None, threads=None, keep_history=False, order=0, store_dtype=np.float64, progress=None):
+def solve(wl, closure=0, fixed_iters=None, threads=None, keep_history=False, order=0, store_dtype=np.float64, progress=None,
+          raytrace_threads=None):
     """Whole hot path for a Workload.  Returns a dict:
          phi     [n_prob][G][nm][cells]  collided flux moments (float64)
          phi_u   [n_src][G][cells]       uncollided scalar flux (zeros for kind 0)
@@ -256,7 +257,9 @@ def solve(wl, closure=0, fixed_iters=None, threads=None, keep_history=False, ord
        groups below).  float64 everywhere except the config-4 goldens (tests/golden/make_goldens.py), where 47 groups
        x 16 moments x 8.4 M cells would take 50 GB per source: float32 there (relative rounding 6e-8, three orders
        below the 1e-4 gate; the iteration of the current group is always float64).
-       progress: None or a callable (problem, group, sweeps, delta) called after every finished group (logging only)."""
+       progress: None or a callable (problem, group, sweeps, delta) called after every finished group (logging only).
+       raytrace_threads: threads of the ray trace alone (default = threads; bench.py times the sweeps on one thread
+       without waiting for a one-thread ray trace; results do not depend on any thread count)."""
     import time
     cells, G, L = wl.cells, wl.G, wl.L
     nm = (L + 1) ** 2
@@ -279,7 +282,7 @@ def solve(wl, closure=0, fixed_iters=None, threads=None, keep_history=False, ord
     Yu = [None] * n_src
     for s, src in enumerate(wl.sources):
         if src.kind in (1, 2, 3):
-            phi_u[s] = raytrace(wl, src, threads=threads)
+            phi_u[s] = raytrace(wl, src, threads=raytrace_threads or threads)
             Yu[s] = real_sph_harm(L, unit_dirs_from(wl, src.pos)).T.copy()        # [nm][cells]
     seconds["raytrace"] = time.perf_counter() - t0
 

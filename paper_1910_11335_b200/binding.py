@@ -23,6 +23,7 @@ EXPORTS = [
     "doctors_set_workspace", "doctors_solve", "doctors_get_flux_moments", "doctors_get_uncollided_flux", "doctors_get_response",
     "doctors_debug_schedule_dims", "doctors_debug_get_schedule", "doctors_debug_device_brick_steps", "doctors_wavefront_size", "doctors_debug_get_tables",
     "doctors_host_level_symmetric", "doctors_host_schedule", "doctors_host_projection_tables",
+    "doctors_host_pl_exceeds_quadrature",
 ]
 
 
@@ -52,7 +53,8 @@ class CSolveInfo(C.Structure):
                 ("ms_iterate", C.c_double), ("ms_total", C.c_double),
                 ("updates", C.c_ulonglong), ("sweep_launches", C.c_ulonglong), ("kernel_launches", C.c_ulonglong),
                 ("n_chunks", C.c_int), ("brick", C.c_int * 3), ("ctas_per_sm", C.c_int),
-                ("sweep_kernel", C.c_int), ("projection_mtiles", C.c_int)]
+                ("sweep_kernel", C.c_int), ("projection_mtiles", C.c_int),
+                ("timed_sweeps", C.c_ulonglong), ("pl_exceeds_quadrature", C.c_int)]
 
 
 _lib = None
@@ -107,6 +109,7 @@ def load_library():
     L.doctors_host_level_symmetric.argtypes = [C.c_int, dp, dp]
     L.doctors_host_schedule.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
     L.doctors_host_projection_tables.argtypes = [C.c_int, C.c_int, dp, dp, dp, dp]
+    L.doctors_host_pl_exceeds_quadrature.argtypes = [C.c_int, C.c_int, dp, dp, dp]
     _lib = L
     return L
 
@@ -149,6 +152,17 @@ def host_projection_tables(L, omega, w):
     if rc != OK:
         raise DoctorsError(rc, "bad table arguments")
     return M, D
+
+
+def host_pl_exceeds_quadrature(L, omega, w):
+    """(flag, defect): does P_L ask for more than the quadrature integrates exactly?  (host code)"""
+    omega = np.ascontiguousarray(omega, dtype=np.float64)
+    w = np.ascontiguousarray(w, dtype=np.float64)
+    d = C.c_double()
+    rc = load_library().doctors_host_pl_exceeds_quadrature(L, len(w), _ptr(omega, C.c_double), _ptr(w, C.c_double), C.byref(d))
+    if rc < 0:
+        raise DoctorsError(INVALID_ARG, "bad arguments")
+    return bool(rc), d.value
 
 
 class Problem:
@@ -299,7 +313,8 @@ class Problem:
                     ms_iterate=info.ms_iterate, ms_total=info.ms_total, updates=int(info.updates),
                     sweep_launches=int(info.sweep_launches), kernel_launches=int(info.kernel_launches),
                     n_chunks=info.n_chunks, brick=tuple(info.brick), ctas_per_sm=info.ctas_per_sm,
-                    projection_mtiles=info.projection_mtiles, sweep_kernel=info.sweep_kernel)
+                    projection_mtiles=info.projection_mtiles, sweep_kernel=info.sweep_kernel,
+                    timed_sweeps=int(info.timed_sweeps), pl_exceeds_quadrature=int(info.pl_exceeds_quadrature))
 
     # ---- get_* ------------------------------------------------------------------------------
     def get_flux_moments(self, problem, group, l_max=0, out=None):

@@ -51,6 +51,28 @@ struct Plan {
     size_t total = 0;
 };
 
+struct SweepLaunch {
+    CUtensorMap tmQ, tmPhi;
+    BrickParams bp;
+    int grid = 0;
+    size_t smem = 0;
+};
+
+// What the device-side set-up (bricked mesh, tables, task list, tensor maps) was built for: a solve re-uses it when
+// nothing of this changed since, so a second solve on unchanged inputs uploads only the fixed sweep counts.
+struct PrepKey {
+    unsigned long long inputs_version = 0;
+    void* ws = nullptr;
+    size_t total = 0;
+    int chunk = 0, B[3] = {0, 0, 0}, MT = 0, sweep_mode = 0, deterministic = 0, closure = 0, ctas_opt = 0;
+    bool operator==(const PrepKey& k) const
+    {
+        return inputs_version == k.inputs_version && ws == k.ws && total == k.total && chunk == k.chunk && B[0] == k.B[0] &&
+               B[1] == k.B[1] && B[2] == k.B[2] && MT == k.MT && sweep_mode == k.sweep_mode && deterministic == k.deterministic &&
+               closure == k.closure && ctas_opt == k.ctas_opt;
+    }
+};
+
 }  // namespace
 
 struct doctors_problem {
@@ -73,6 +95,20 @@ struct doctors_problem {
     // workspace
     void* ws = nullptr;
     size_t ws_bytes = 0;
+    unsigned long long inputs_version = 1;   // bumped by every set_* call
+    // device-side set-up, cached between solves (prepare())
+    bool prepared = false;
+    PrepKey prep_key;
+    MeshDev md;                              // with pitch and origin (the ray tracer, the fixed source)
+    SweepLaunch SL;
+    std::vector<int> oct_begin;              // slices of the task list (one per launch of an iteration)
+    std::vector<std::vector<int32_t>> sched_off;   // sweep_mode 1: plane offsets per octant
+    int ctas_per_sm = 0;
+    unsigned epoch = 0;                      // "brick done" value of the last sweep launch; grows across solves
+    int pl_inexact = 0;                      // the quadrature does not integrate Y_lm Y_l'm' exactly up to the P_L order set
+    std::vector<cudaEvent_t> ev_pool;        // timing events, owned by the handle (no leak on an error return)
+    size_t ev_used = 0;
+    int* h_flag = nullptr;                   // pinned word for the convergence flag
     // result bookkeeping
     bool solved = false;
     Plan plan;
@@ -105,6 +141,32 @@ int fail(doctors_problem* p, int code, const char* fmt, ...)
 
 int nprob_of(const doctors_problem* p) { return p->mode == 0 ? int(p->sources.size()) : 1; }
 
+// max | sum_n w_n Y_lm (2l'+1)/(4 pi) Y_l'm' - delta | over all moment pairs up to P_L (Galerkin identity D^T M = I)
+double galerkin_defect(int L, const std::vector<double>& omega, const std::vector<double>& w)
+{
+    std::vector<double> Mt, Dt;
+    projection_tables(L, omega, w, Mt, Dt);
+    const int NM = (L + 1) * (L + 1), nd = int(w.size());
+    double worst = 0.0;
+    for (int a = 0; a < NM; ++a)
+        for (int b = 0; b < NM; ++b) {
+            double acc = 0.0;
+            for (int n = 0; n < nd; ++n) acc += Dt[size_t(n) * NM + a] * Mt[size_t(n) * NM + b];
+            worst = std::max(worst, std::fabs(acc - (a == b ? 1.0 : 0.0)));
+        }
+    return worst;
+}
+constexpr double kGalerkinTol = 1e-9;
+
+// projection = 2: tensor cores where they apply; 0 (automatic): tensor cores for more than 16 directions per octant
+// (S12, S16: measured on config 3, S16 P3, 619.6 against 730.3 ms per solve), the FMA loops below (config 4, S8: 4-7 %
+// faster than the tensor-core path); 1: always the FMA loops.
+bool wants_mma(const doctors_solve_opts* o, int M)
+{
+    const int pr = o ? o->projection : 0;
+    return pr == 2 || (pr == 0 && M > 16);
+}
+
 void auto_brick(int NM, int M, int nx, int ny, int nz, const int* req, bool mt, int B[3])
 {
     if (req && req[0] > 0 && req[1] > 0 && req[2] > 0) { B[0] = req[0]; B[1] = req[1]; B[2] = req[2]; return; }
@@ -113,10 +175,20 @@ void auto_brick(int NM, int M, int nx, int ny, int nz, const int* req, bool mt, 
     B[2] = std::min(32 / B[1], nz);
     if (B[2] < 4 && B[1] < ny) B[1] = std::min(32 / B[2], ny);
     const int cand[5] = {20, 16, 12, 8, 4};        // 20 x 8 x 4 = 640 cells = 2 per thread of a 320-thread CTA, 3 CTAs per SM
+    auto fits = [&](int bx, size_t limit) {
+        return brick_smem_layout(NM, bx, B[1], B[2], M, mt ? projection_mtiles(NM, M, bx * B[1] * B[2]) : 0).total <= limit;
+    };
     for (int c = 0; c < 5; ++c) {
         B[0] = std::min(cand[c], (nx + 3) / 4 * 4);
-        if (brick_smem_layout(NM, B[0], B[1], B[2], M, mt ? projection_mtiles(NM, M, B[0] * B[1] * B[2]) : 0).total <= 74 * 1024) break;
+        if (fits(B[0], 74 * 1024)) break;
     }
+    // many directions per octant (S16: 36 planes per tile): a brick shorter than 8 cells leaves 70 % of the wavefront's
+    // lane-steps idle; two CTAs per SM with 8-cell bricks are faster (config 3: 2.86 against 3.47 ms per sweep)
+    if (B[0] < 8 && nx > 4)
+        for (int c = 0; c < 5; ++c) {
+            const int bx = std::min(cand[c], (nx + 3) / 4 * 4);
+            if (fits(bx, 113 * 1024)) { B[0] = bx; break; }
+        }
 }
 
 // Lay out the workspace.  chunk = problems solved together.
@@ -133,7 +205,7 @@ Plan make_plan(const doctors_problem* p, const doctors_solve_opts* o, int chunk)
     P.sweep_mode = o ? o->sweep_mode : 0;
     P.deterministic = o ? o->deterministic : 0;
     for (auto& s : p->sources) if (s.kind == 0) ++P.nvol;
-    auto_brick(P.NM, P.M, p->nx, p->ny, p->nz, o ? o->brick : nullptr, o && o->projection == 2, P.B);
+    auto_brick(P.NM, P.M, p->nx, p->ny, p->nz, o ? o->brick : nullptr, wants_mma(o, P.M), P.B);
     P.gb[0] = (p->nx + P.B[0] - 1) / P.B[0];
     P.gb[1] = (p->ny + P.B[1] - 1) / P.B[1];
     P.gb[2] = (p->nz + P.B[2] - 1) / P.B[2];
@@ -145,7 +217,7 @@ Plan make_plan(const doctors_problem* p, const doctors_solve_opts* o, int chunk)
     while ((P.NCb / 4) % P.tm_rows != 0 || P.NCb / P.tm_rows > 256) ++P.tm_rows;
     P.tm_inner = P.NCb / P.tm_rows;
     P.ntasks = P.nbricks * 8 * P.chunk;
-    P.MT = (o && o->projection == 2) ? projection_mtiles(P.NM, P.M, P.NCb) : 0;
+    P.MT = wants_mma(o, P.M) ? projection_mtiles(P.NM, P.M, P.NCb) : 0;
     P.smem = brick_smem_layout(P.NM, P.B[0], P.B[1], P.B[2], P.M, P.MT).total;
     { int dpw = (P.M + kMaxSweepWarps - 1) / kMaxSweepWarps; P.W = (P.M + dpw - 1) / dpw; }
 
@@ -278,7 +350,13 @@ int doctors_create_problem(int cuda_device, void* stream, doctors_problem** out)
     return DOCTORS_OK;
 }
 
-void doctors_destroy_problem(doctors_problem* p) { delete p; }
+void doctors_destroy_problem(doctors_problem* p)
+{
+    if (!p) return;
+    for (cudaEvent_t e : p->ev_pool) cudaEventDestroy(e);
+    if (p->h_flag) cudaFreeHost(p->h_flag);
+    delete p;
+}
 
 const char* doctors_last_error(const doctors_problem* p) { return p ? p->err.c_str() : "null handle"; }
 
@@ -305,6 +383,7 @@ int doctors_set_mesh_materials(doctors_problem* p, int nx, int ny, int nz, doubl
     if (density) p->rho.assign(density, density + cells); else p->rho.assign(cells, 1.0f);
     p->has_mesh = true;
     p->solved = false;
+    ++p->inputs_version;
     return DOCTORS_OK;
 }
 
@@ -334,6 +413,7 @@ int doctors_set_xs(doctors_problem* p, int n_materials, int n_groups, int pl_ord
     p->sigs.assign(sigma_s, sigma_s + size_t(n_materials) * (L + 1) * G * G);
     p->has_xs = true;
     p->solved = false;
+    ++p->inputs_version;
     return DOCTORS_OK;
 }
 
@@ -346,6 +426,7 @@ int doctors_set_quadrature(doctors_problem* p, int sn_order)
     p->omega = om; p->w = w; p->ndir = int(w.size());
     p->has_quad = true;
     p->solved = false;
+    ++p->inputs_version;
     return DOCTORS_OK;
 }
 
@@ -378,6 +459,7 @@ int doctors_set_quadrature_points(doctors_problem* p, int n_dir, const double* o
     p->ndir = n_dir;
     p->has_quad = true;
     p->solved = false;
+    ++p->inputs_version;
     return DOCTORS_OK;
 }
 
@@ -447,6 +529,7 @@ int doctors_set_source(doctors_problem* p, int n_sources, const doctors_source* 
     p->mode = mode;
     p->has_src = true;
     p->solved = false;
+    ++p->inputs_version;
     return DOCTORS_OK;
 }
 
@@ -469,6 +552,7 @@ int doctors_set_workspace(doctors_problem* p, void* device_ptr, size_t bytes)
     if (!device_ptr || (reinterpret_cast<uintptr_t>(device_ptr) & 255u)) return fail(p, DOCTORS_INVALID_ARG, "workspace must be non-NULL and 256-byte aligned");
     p->ws = device_ptr; p->ws_bytes = bytes;
     p->solved = false;
+    ++p->inputs_version;
     return DOCTORS_OK;
 }
 
@@ -481,7 +565,7 @@ int doctors_debug_schedule_dims(doctors_problem* p, const doctors_solve_opts* op
     if (level == 0) { dims[0] = p->nx; dims[1] = p->ny; dims[2] = p->nz; return DOCTORS_OK; }
     if (!p->has_xs || !p->has_quad) return fail(p, DOCTORS_BAD_STATE, "xs / quadrature not set (brick size depends on them)");
     int B[3];
-    auto_brick((p->L + 1) * (p->L + 1), p->ndir / 8, p->nx, p->ny, p->nz, opts ? opts->brick : nullptr, opts && opts->projection == 2, B);
+    auto_brick((p->L + 1) * (p->L + 1), p->ndir / 8, p->nx, p->ny, p->nz, opts ? opts->brick : nullptr, wants_mma(opts, p->ndir / 8), B);
     if (level == 1) { for (int a = 0; a < 3; ++a) dims[a] = ((a == 0 ? p->nx : a == 1 ? p->ny : p->nz) + B[a] - 1) / B[a]; return DOCTORS_OK; }
     if (level == 2) { for (int a = 0; a < 3; ++a) dims[a] = B[a]; return DOCTORS_OK; }
     return fail(p, DOCTORS_INVALID_ARG, "level must be 0, 1 or 2");
@@ -529,6 +613,15 @@ int doctors_host_schedule(int nx, int ny, int nz, int octant, int32_t* plane_off
     std::memcpy(plane_offset, off.data(), off.size() * 4);
     std::memcpy(cell_of, cells.data(), cells.size() * 4);
     return DOCTORS_OK;
+}
+
+int doctors_host_pl_exceeds_quadrature(int pl_order, int n_dir, const double* omega_xyz, const double* w, double* defect)
+{
+    if (pl_order < 0 || pl_order > 3 || n_dir <= 0 || !omega_xyz || !w) return -1;
+    std::vector<double> om(omega_xyz, omega_xyz + 3 * size_t(n_dir)), ww(w, w + n_dir);
+    const double d = galerkin_defect(pl_order, om, ww);
+    if (defect) *defect = d;
+    return d > kGalerkinTol ? 1 : 0;
 }
 
 int doctors_host_projection_tables(int pl_order, int n_dir, const double* omega_xyz, const double* w, double* Mtab, double* Dtab)
@@ -599,13 +692,6 @@ int make_tensor_map(doctors_problem* p, CUtensorMap* tm, void* base, int rank, c
     if (r != CUDA_SUCCESS) return fail(p, DOCTORS_CUDA, "cuTensorMapEncodeTiled failed (%d)", int(r));
     return DOCTORS_OK;
 }
-
-struct SweepLaunch {
-    CUtensorMap tmQ, tmPhi;
-    BrickParams bp;
-    int grid = 0;
-    size_t smem = 0;
-};
 
 template <int NM, bool FIX, int MT>
 cudaError_t launch_brick(const SweepLaunch& S, cudaStream_t st)
@@ -701,40 +787,14 @@ std::vector<unsigned char> build_octtabs(int NM, int M, int MT, const std::vecto
     return blob;
 }
 
-}  // namespace
-
-extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_in, doctors_solve_info* info)
+// Device-side set-up for one plan: inputs in brick-major order, tables, task list (a3), tensor maps.  Runs when an
+// input, the workspace or a layout option changed (PrepKey); doctors_solve itself then only enqueues kernels.
+int prepare(doctors_problem* p, const doctors_solve_opts& o, const Plan& P)
 {
-    if (!p) return DOCTORS_INVALID_ARG;
-    int rc = check_ready(p);
-    if (rc != DOCTORS_OK) return rc;
-    doctors_solve_opts o;
-    std::memset(&o, 0, sizeof o);
-    if (opts_in) o = *opts_in;
-    if (!(o.tol > 0.0)) o.tol = 1e-5;
-    if (o.max_iters <= 0) o.max_iters = 100;
-    const bool adaptive_window = o.check_window <= 0;   // first host read where the previous group stopped, then every sweep
-    if (o.check_window <= 0) o.check_window = 12;
-    if (o.closure != 0 && o.closure != 1) return fail(p, DOCTORS_INVALID_ARG, "closure must be 0 or 1");
-    if (o.sweep_mode < 0 || o.sweep_mode > 1) return fail(p, DOCTORS_INVALID_ARG, "sweep_mode must be 0 or 1");
-    if (o.brick[0] > 0 && (o.brick[0] % 4 != 0 || o.brick[0] > 64 || o.brick[1] <= 0 || o.brick[2] <= 0 || o.brick[1] * o.brick[2] > 32))
-        return fail(p, DOCTORS_INVALID_ARG, "brick: brick[0] a multiple of 4 (<= 64), brick[1] * brick[2] <= 32 (the lanes of a warp)");
-    if (!p->ws) return fail(p, DOCTORS_ALLOC, "no workspace set");
-    CK(cudaSetDevice(p->device));
     cudaStream_t st = p->stream;
-
-    const int chunk = choose_chunk(p, &o, p->ws_bytes);
-    Plan P = make_plan(p, &o, chunk);
-    if (P.total > p->ws_bytes)
-        return fail(p, DOCTORS_ALLOC, "workspace too small: need %zu bytes (chunk %d), have %zu", P.total, P.chunk, p->ws_bytes);
-    if (P.chunk > 255) return fail(p, DOCTORS_INVALID_ARG, "chunk too large");
-    if (P.gb[0] > 1023 || P.gb[1] > 1023 || P.gb[2] > 1023) return fail(p, DOCTORS_INVALID_ARG, "brick grid too large");
-    p->solved = false;
-    p->plan = P;
     const int NM = P.NM, G = P.G, L = P.L, M = P.M;
     const size_t cp = size_t(P.cells_p);
     const int nx = p->nx, ny = p->ny, nz = p->nz;
-
     MeshDev md;
     md.nx = nx; md.ny = ny; md.nz = nz; md.cells_p = P.cells_p;
     md.BX = P.B[0]; md.BY = P.B[1]; md.BZ = P.B[2]; md.gbx = P.gb[0]; md.gby = P.gb[1]; md.gbz = P.gb[2]; md.NCb = P.NCb;
@@ -798,8 +858,6 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
                              float(p->w[n] * std::fabs(p->omega[3 * n + 1]) * p->dx * p->dz),
                              float(p->w[n] * std::fabs(p->omega[3 * n + 2]) * p->dx * p->dy), 0.0f);
     }
-    std::vector<int> fixed_h(size_t(P.nprob) * G, 0);
-    if (o.fixed_iters) std::copy(o.fixed_iters, o.fixed_iters + fixed_h.size(), fixed_h.begin());
     CK(cudaMemcpyAsync(at<double>(p, P.o_sigt_hat), p->sigt.data(), p->sigt.size() * 8, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(at<float>(p, P.o_sigs), sigs_f.data(), sigs_f.size() * 4, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(at<double>(p, P.o_spec), spec.data(), spec.size() * 8, cudaMemcpyHostToDevice, st));
@@ -808,14 +866,17 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
     CK(cudaMemcpyAsync(at<float>(p, P.o_dtab), Dt_f.data(), Dt_f.size() * 4, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(at<double>(p, P.o_dird), dird.data(), dird.size() * 8, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(at<float4>(p, P.o_lk), lkc.data(), lkc.size() * 16, cudaMemcpyHostToDevice, st));
-    CK(cudaMemcpyAsync(at<int>(p, P.o_fixediters), fixed_h.data(), fixed_h.size() * 4, cudaMemcpyHostToDevice, st));
 
     // ---- schedules (a3) ----
     std::vector<uint2> tasks;
-    std::vector<int> oct_begin(9, 0);
-    std::vector<std::vector<int32_t>> sched_off(8);
-    SweepLaunch SL;
-    int ctas_per_sm = 0;
+    std::vector<int>& oct_begin = p->oct_begin;
+    oct_begin.assign(9, 0);
+    std::vector<std::vector<int32_t>>& sched_off = p->sched_off;
+    sched_off.assign(8, std::vector<int32_t>());
+    SweepLaunch& SL = p->SL;
+    int& ctas_per_sm = p->ctas_per_sm;
+    ctas_per_sm = 0;
+    int rc = DOCTORS_OK;
     if (P.sweep_mode == 0) {
         // level 2 (cells of a brick) needs no table: lane (j',k') at step s updates i' = s - j' - k' (Eq. 8)
         // level 1: bricks in sub-sweep order of the brick grid, per octant
@@ -863,7 +924,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
             CK(cudaStreamSynchronize(st));
         }
         int max_ctas = 0;
-        cudaError_t e;
+        cudaError_t e = cudaSuccess;
         DISPATCH_NM_FIX(NM, o.closure == 1, P.MT, e = (prep_brick<NM, FIX, MT>(P.smem, 32 * P.W, &max_ctas)));
         if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "sweep kernel setup failed: %s (smem %zu)", cudaGetErrorString(e), P.smem);
         if (max_ctas < 1) return fail(p, DOCTORS_CUDA, "sweep kernel does not fit an SM (smem %zu)", P.smem);
@@ -894,22 +955,114 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
             CK(cudaStreamSynchronize(st));
         }
     }
-    CK(cudaStreamSynchronize(st));     // host staging vectors may go out of scope from here on
+    CK(cudaStreamSynchronize(st));     // host staging vectors go out of scope here
+    p->md = md;
+    p->epoch = 0;                      // the flags were just cleared
+    // Does the quadrature integrate the products Y_lm Y_l'm' exactly up to the P_L order set?  (Galerkin identity:
+    // sum_n w_n Y_lm (2l'+1)/(4 pi) Y_l'm' = delta.  Level-symmetric sets: exact up to P1/P2/P3/P4 at S2/S4/S6/S8, >= P5 at
+    // S12/S16, DESIGN.md App. A; a higher P_L still runs, the moments of the scattering source are then inconsistent.)
+    p->pl_inexact = galerkin_defect(L, p->omega, p->w) > kGalerkinTol ? 1 : 0;
+    return DOCTORS_OK;
+}
 
-    // ---- events ----
-    cudaEvent_t ev_total0, ev_total1, ev_a, ev_b;
-    CK(cudaEventCreate(&ev_total0)); CK(cudaEventCreate(&ev_total1)); CK(cudaEventCreate(&ev_a)); CK(cudaEventCreate(&ev_b));
-    std::vector<cudaEvent_t> sweep_ev;       // pairs
-    std::vector<cudaEvent_t> fixed_ev, iter_ev;
-    auto new_event = [&](std::vector<cudaEvent_t>& v) { cudaEvent_t e; cudaEventCreate(&e); v.push_back(e); return e; };
+
+}  // namespace
+
+extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_in, doctors_solve_info* info)
+{
+    if (!p) return DOCTORS_INVALID_ARG;
+    int rc = check_ready(p);
+    if (rc != DOCTORS_OK) return rc;
+    doctors_solve_opts o;
+    std::memset(&o, 0, sizeof o);
+    if (opts_in) o = *opts_in;
+    if (!(o.tol > 0.0)) o.tol = 1e-5;
+    if (o.max_iters <= 0) o.max_iters = 100;
+    const bool adaptive_window = o.check_window <= 0;   // first host read where the previous group stopped, then every sweep
+    if (o.check_window <= 0) o.check_window = 12;
+    if (o.closure != 0 && o.closure != 1) return fail(p, DOCTORS_INVALID_ARG, "closure must be 0 or 1");
+    if (o.sweep_mode < 0 || o.sweep_mode > 1) return fail(p, DOCTORS_INVALID_ARG, "sweep_mode must be 0 or 1");
+    if (o.brick[0] > 0 && (o.brick[0] % 4 != 0 || o.brick[0] > 64 || o.brick[1] <= 0 || o.brick[2] <= 0 || o.brick[1] * o.brick[2] > 32))
+        return fail(p, DOCTORS_INVALID_ARG, "brick: brick[0] a multiple of 4 (<= 64), brick[1] * brick[2] <= 32 (the lanes of a warp)");
+    if (!p->ws) return fail(p, DOCTORS_ALLOC, "no workspace set");
+    CK(cudaSetDevice(p->device));
+    cudaStream_t st = p->stream;
+
+    const int chunk = choose_chunk(p, &o, p->ws_bytes);
+    Plan P = make_plan(p, &o, chunk);
+    if (P.total > p->ws_bytes)
+        return fail(p, DOCTORS_ALLOC, "workspace too small: need %zu bytes (chunk %d), have %zu", P.total, P.chunk, p->ws_bytes);
+    if (P.chunk > 255) return fail(p, DOCTORS_INVALID_ARG, "chunk too large");
+    if (P.gb[0] > 1023 || P.gb[1] > 1023 || P.gb[2] > 1023) return fail(p, DOCTORS_INVALID_ARG, "brick grid too large");
+    p->solved = false;
+    p->plan = P;
+    const int NM = P.NM, G = P.G, L = P.L, M = P.M;
+    const size_t cp = size_t(P.cells_p);
+    const int nx = p->nx, ny = p->ny, nz = p->nz;
+    if (size_t(p->n_mat_xs) * (L + 1) * G * 4 > 200 * 1024)
+        return fail(p, DOCTORS_INVALID_ARG, "scattering rows of one destination group (n_materials x (L+1) x G floats = %zu bytes) "
+                    "do not fit the fixed-source kernel's shared memory (200 KB)", size_t(p->n_mat_xs) * (L + 1) * G * 4);
+
+    PrepKey key;
+    key.inputs_version = p->inputs_version; key.ws = p->ws; key.total = P.total; key.chunk = P.chunk;
+    key.B[0] = P.B[0]; key.B[1] = P.B[1]; key.B[2] = P.B[2]; key.MT = P.MT; key.sweep_mode = P.sweep_mode;
+    key.deterministic = P.deterministic; key.closure = o.closure; key.ctas_opt = o.ctas_per_sm;
+    if (!p->prepared || !(p->prep_key == key)) {
+        p->prepared = false;
+        rc = prepare(p, o, P);
+        if (rc != DOCTORS_OK) return rc;
+        p->prepared = true;
+        p->prep_key = key;
+    }
+    const MeshDev md = p->md;
+    SweepLaunch& SL = p->SL;
+    const std::vector<int>& oct_begin = p->oct_begin;
+    const std::vector<std::vector<int32_t>>& sched_off = p->sched_off;
+    const int ctas_per_sm = p->ctas_per_sm;
+    std::vector<int> fixed_h(size_t(P.nprob) * G, 0);
+    if (o.fixed_iters) std::copy(o.fixed_iters, o.fixed_iters + fixed_h.size(), fixed_h.begin());
+    CK(cudaMemcpyAsync(at<int>(p, P.o_fixediters), fixed_h.data(), fixed_h.size() * 4, cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st));           // fixed_h is pageable: the copy is staged, but do not rely on it
+
+    // ---- events: a pool owned by the handle; every sweep launch is timed, however long the solve ----
+    p->ev_used = 0;
+    cudaError_t ev_err = cudaSuccess;
+    auto next_event = [&]() -> cudaEvent_t {
+        if (p->ev_used == p->ev_pool.size()) {
+            cudaEvent_t e = nullptr;
+            cudaError_t ce = cudaEventCreate(&e);
+            if (ce != cudaSuccess) { ev_err = ce; return nullptr; }
+            p->ev_pool.push_back(e);
+        }
+        return p->ev_pool[p->ev_used++];
+    };
+#define NEXT_EVENT(var)                                                                                      \
+    cudaEvent_t var = next_event();                                                                          \
+    if (!var) return fail(p, DOCTORS_CUDA, "cudaEventCreate failed: %s", cudaGetErrorString(ev_err))
+    NEXT_EVENT(ev_total0); NEXT_EVENT(ev_total1); NEXT_EVENT(ev_a); NEXT_EVENT(ev_b);
+    std::vector<cudaEvent_t> sweep_ev, fixed_ev, iter_ev;       // pairs (the events themselves live in the pool)
     double ms_ray = 0.0;
     unsigned long long sweep_launches = 0, kernel_launches = 0, updates = 0;
-    unsigned epoch = 0;
-    int* h_flag = nullptr;
-    CK(cudaMallocHost(&h_flag, 64));
+    unsigned& epoch = p->epoch;
+    if (!p->h_flag) CK(cudaMallocHost(&p->h_flag, 64));
+    int* h_flag = p->h_flag;
     bool not_converged = false;
     const unsigned cblocks = unsigned((P.cells_p + 255) / 256);
     const int red_blocks = int(std::min<long long>((P.cells_p + 255) / 256, 4LL * p->num_sms));
+    {
+        // the fixed-source kernel stages the scattering rows of the destination group in shared memory
+        const size_t need = size_t(p->n_mat_xs) * (L + 1) * G * 4;
+        if (need > 48 * 1024) {
+            cudaError_t e = cudaSuccess;
+            switch (NM) {
+                case 1: e = cudaFuncSetAttribute(k_fixed_source<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(need)); break;
+                case 4: e = cudaFuncSetAttribute(k_fixed_source<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(need)); break;
+                case 9: e = cudaFuncSetAttribute(k_fixed_source<9>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(need)); break;
+                default: e = cudaFuncSetAttribute(k_fixed_source<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(need)); break;
+            }
+            if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "fixed-source kernel setup failed: %s", cudaGetErrorString(e));
+        }
+    }
 
     CK(cudaEventRecord(ev_total0, st));
     for (int ch = 0; ch < P.nchunks; ++ch) {
@@ -935,7 +1088,8 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
             k_group_begin<<<1, 256, 0, st>>>(at<ProbState>(p, P.o_state), at<Control>(p, P.o_ctl), at<int>(p, P.o_fixediters),
                                               prob0, nq, P.chunk, G, g, at<double>(p, P.o_bal));
             k_sigt<<<cblocks, 256, 0, st>>>(md, at<uint8_t>(p, P.o_mat), at<float>(p, P.o_rho), at<double>(p, P.o_sigt_hat), G, g, at<double>(p, P.o_sigt));
-            cudaEvent_t f0 = new_event(fixed_ev), f1 = new_event(fixed_ev);
+            NEXT_EVENT(f0); NEXT_EVENT(f1);
+            fixed_ev.push_back(f0); fixed_ev.push_back(f1);
             CK(cudaEventRecord(f0, st));
             {
                 size_t sm = size_t(p->n_mat_xs) * (L + 1) * (g + 1) * 4;
@@ -958,7 +1112,8 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
                 max_fixed = std::max(max_fixed, f);
             }
             const int limit = all_fixed ? max_fixed : std::max(o.max_iters, max_fixed);
-            cudaEvent_t i0 = new_event(iter_ev), i1 = new_event(iter_ev);
+            NEXT_EVENT(i0); NEXT_EVENT(i1);
+            iter_ev.push_back(i0); iter_ev.push_back(i1);
             CK(cudaEventRecord(i0, st));
             int k = 0;
             while (k < limit) {
@@ -973,8 +1128,9 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
                     switch (NM) { case 1: LAUNCH_UPDATE(1); break; case 4: LAUNCH_UPDATE(4); break; case 9: LAUNCH_UPDATE(9); break; default: LAUNCH_UPDATE(16); }
 #undef LAUNCH_UPDATE
                     ++kernel_launches;
-                    cudaEvent_t s0 = nullptr, s1 = nullptr;
-                    if (sweep_ev.size() < 16384) { s0 = new_event(sweep_ev); s1 = new_event(sweep_ev); CK(cudaEventRecord(s0, st)); }
+                    NEXT_EVENT(s0); NEXT_EVENT(s1);
+                    sweep_ev.push_back(s0); sweep_ev.push_back(s1);
+                    CK(cudaEventRecord(s0, st));
                     if (P.sweep_mode == 0) {
                         SL.bp.g = g;
                         const int nl = P.deterministic ? 8 : 1;
@@ -1007,7 +1163,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
                                 ++sweep_launches; ++kernel_launches;
                             }
                     }
-                    if (s1) CK(cudaEventRecord(s1, st));
+                    CK(cudaEventRecord(s1, st));
                     k_check<<<dim3(red_blocks, nq), 256, 0, st>>>(md, g, G, NM, at<float>(p, P.o_phiall), at<float>(p, P.o_phi0old),
                                                                    at<ProbState>(p, P.o_state), at<Control>(p, P.o_ctl), nq, float(o.tol), o.max_iters);
                     ++kernel_launches;
@@ -1065,12 +1221,10 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         info->ctas_per_sm = ctas_per_sm;
         info->projection_mtiles = P.sweep_mode == 0 ? P.MT : 0;
         info->sweep_kernel = o.sweep_mode == 1 ? 1 : 0;
+        info->timed_sweeps = (unsigned long long)(sweep_ev.size() / 2);
+        info->pl_exceeds_quadrature = p->pl_inexact;
     }
-    for (auto e : sweep_ev) cudaEventDestroy(e);
-    for (auto e : fixed_ev) cudaEventDestroy(e);
-    for (auto e : iter_ev) cudaEventDestroy(e);
-    cudaEventDestroy(ev_total0); cudaEventDestroy(ev_total1); cudaEventDestroy(ev_a); cudaEventDestroy(ev_b);
-    cudaFreeHost(h_flag);
+#undef NEXT_EVENT
     p->solved = true;
     if (not_converged) { p->err = "some (problem, group) stopped at max_iters"; return DOCTORS_NOT_CONVERGED; }
     return DOCTORS_OK;

@@ -46,7 +46,8 @@ def test_struct_layouts_match_the_library(pkg):
     from paper_1910_11335_b200 import binding
     assert tuple(sizes) == (ctypes.sizeof(binding.CSource), ctypes.sizeof(binding.CSolveOpts), ctypes.sizeof(binding.CSolveInfo))
     assert [f[0] for f in binding.CSolveOpts._fields_][-2:] == ["check_window", "projection"]
-    assert [f[0] for f in binding.CSolveInfo._fields_][-2:] == ["sweep_kernel", "projection_mtiles"]
+    assert [f[0] for f in binding.CSolveInfo._fields_][-4:] == ["sweep_kernel", "projection_mtiles", "timed_sweeps",
+                                                                "pl_exceeds_quadrature"]
 
 
 def test_version_and_no_device_error(pkg):
@@ -124,3 +125,16 @@ def test_source_files_do_not_name_forbidden_calls():
         for f in files:
             if f.endswith((".py", ".cu", ".cuh", ".h", ".cpp", ".c")):
                 assert not bad.search(open(os.path.join(base, f), errors="ignore").read()), f
+
+
+def test_pl_vs_sn_exactness_warning(pkg):
+    """level-symmetric sets integrate Y_lm Y_l'm' exactly up to P1 / P2 / P3 / P4 at S2 / S4 / S6 / S8 and at
+    least P3 at S12 / S16; one order higher fails at the 0.1-5 level.  The library flags a P_L that asks for more."""
+    from paper_1910_11335_b200 import binding
+    exact_up_to = {2: 1, 4: 2, 6: 3, 8: 3, 12: 3, 16: 3}            # the library stops at P3
+    for N, Lmax in exact_up_to.items():
+        om, w = binding.host_level_symmetric(N)
+        for L in range(4):
+            flag, defect = binding.host_pl_exceeds_quadrature(L, om, w)
+            assert flag == (L > Lmax), (N, L, defect)
+            assert defect < 1e-12 if L <= Lmax else defect > 0.05, (N, L, defect)
