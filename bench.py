@@ -220,8 +220,7 @@ def bench_config(wl, args, info):
                else "working set fits L2; an L2 flush (256 MiB write) runs between steps",
          "parallelism": "replicas only" if args.gpus > 1 else "1 GPU"}
     if info is not None:
-        c.update({"source_chunks": info["n_chunks"], "brick": list(info["brick"]), "ctas_per_sm": info["ctas_per_sm"],
-                  "tile_buffers": info["tile_buffers"]})
+        c.update({"source_chunks": info["n_chunks"], "brick": list(info["brick"]), "ctas_per_sm": info["ctas_per_sm"]})
     return c
 
 
@@ -271,8 +270,6 @@ def run_gpu_arm(args):
         kw["brick"] = tuple(int(v) for v in args.brick.split(","))
     if args.ctas:
         kw["ctas_per_sm"] = args.ctas
-    if args.tile_buffers:
-        kw["tile_buffers"] = args.tile_buffers
     flush = None
     if wl.cells * 33 * 4 * min(4, len(wl.sources)) <= 126e6:
         flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
@@ -394,7 +391,6 @@ def main():
     ap.add_argument("--slice", action="store_true", help="profiling slice of the config (see workload_for); not a bench number")
     ap.add_argument("--projection", type=int, default=0, help="doctors_solve_opts.projection (experiments; 0 = the library's default)")
     ap.add_argument("--brick", default="", help="bx,by,bz brick extents (experiments; default automatic)")
-    ap.add_argument("--tile-buffers", type=int, default=0, help="doctors_solve_opts.tile_buffers (experiments; 0 = automatic)")
     ap.add_argument("--ctas", type=int, default=0, help="persistent CTAs per SM (experiments; default occupancy maximum)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")

@@ -125,8 +125,6 @@ typedef struct {
                                *   (the faster of the two as measured on B200); 1 packed fp32 FMA loops;
                                * 2 tensor cores (mma TF32, 3-product split, fp32 accumulate) when P3, <= 48 directions per
                                *   octant and a brick of a multiple of 8 cells; else the FMA loops */
-    int tile_buffers;         /* sweep_mode 0: 0 automatic; 2 = software-pipelined kernel (the next brick's Q tile is loaded while
-                               * this one is swept, two CTAs per SM; FMA-loop projections only); 1 = one tile, three CTAs per SM */
 } doctors_solve_opts;
 
 typedef struct {
@@ -142,7 +140,6 @@ typedef struct {
     int ctas_per_sm;
     int sweep_kernel;         /* kernel that swept: 0 brick, 1 paper scheme */
     int projection_mtiles;    /* > 0: the projections ran on the tensor cores (16-direction m-tiles per octant); 0: fp32 FMA loops */
-    int tile_buffers;         /* tile buffers the sweep kernel ran with (1 or 2; 0 for sweep_mode 1) */
     unsigned long long timed_sweeps;   /* sweep iterations whose CUDA-event time is in ms_sweep (= all of them) */
     int pl_exceeds_quadrature;/* warning flag: 1 if the quadrature does not integrate Y_lm Y_l'm' exactly up to pl_order
                                * (level-symmetric sets: exact up to P1 / P2 / P3 / P4 at S2 / S4 / S6 / S8, >= P5 at S12 / S16;

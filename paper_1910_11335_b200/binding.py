@@ -43,7 +43,7 @@ class CSolveOpts(C.Structure):
     _fields_ = [("tol", C.c_double), ("max_iters", C.c_int), ("fixed_iters", C.POINTER(C.c_int)),
                 ("closure", C.c_int), ("deterministic", C.c_int), ("source_chunk", C.c_int),
                 ("sweep_mode", C.c_int), ("brick", C.c_int * 3), ("ctas_per_sm", C.c_int),
-                ("check_window", C.c_int), ("projection", C.c_int), ("tile_buffers", C.c_int)]
+                ("check_window", C.c_int), ("projection", C.c_int)]
 
 
 class CSolveInfo(C.Structure):
@@ -53,7 +53,7 @@ class CSolveInfo(C.Structure):
                 ("ms_iterate", C.c_double), ("ms_total", C.c_double),
                 ("updates", C.c_ulonglong), ("sweep_launches", C.c_ulonglong), ("kernel_launches", C.c_ulonglong),
                 ("n_chunks", C.c_int), ("brick", C.c_int * 3), ("ctas_per_sm", C.c_int),
-                ("sweep_kernel", C.c_int), ("projection_mtiles", C.c_int), ("tile_buffers", C.c_int),
+                ("sweep_kernel", C.c_int), ("projection_mtiles", C.c_int),
                 ("timed_sweeps", C.c_ulonglong), ("pl_exceeds_quadrature", C.c_int)]
 
 
@@ -266,12 +266,11 @@ class Problem:
 
     # ---- solve ------------------------------------------------------------------------------
     def _opts(self, tol=1e-5, max_iters=100, fixed_iters=None, closure=0, deterministic=0, source_chunk=0,
-              sweep_mode=0, brick=None, ctas_per_sm=0, check_window=0, projection=0, tile_buffers=0):
+              sweep_mode=0, brick=None, ctas_per_sm=0, check_window=0, projection=0):
         o = CSolveOpts()
         o.tol, o.max_iters, o.closure, o.deterministic = tol, max_iters, closure, deterministic
         o.source_chunk, o.sweep_mode, o.ctas_per_sm, o.check_window = source_chunk, sweep_mode, ctas_per_sm, check_window
         o.projection = projection
-        o.tile_buffers = tile_buffers
         if brick is not None:
             o.brick = (C.c_int * 3)(*brick)
         fi = None
@@ -315,7 +314,7 @@ class Problem:
                     sweep_launches=int(info.sweep_launches), kernel_launches=int(info.kernel_launches),
                     n_chunks=info.n_chunks, brick=tuple(info.brick), ctas_per_sm=info.ctas_per_sm,
                     projection_mtiles=info.projection_mtiles, sweep_kernel=info.sweep_kernel,
-                    tile_buffers=info.tile_buffers, timed_sweeps=int(info.timed_sweeps), pl_exceeds_quadrature=int(info.pl_exceeds_quadrature))
+                    timed_sweeps=int(info.timed_sweeps), pl_exceeds_quadrature=int(info.pl_exceeds_quadrature))
 
     # ---- get_* ------------------------------------------------------------------------------
     def get_flux_moments(self, problem, group, l_max=0, out=None):

@@ -36,7 +36,6 @@ struct Plan {
     bool ok = false;
     long long cells_p = 0; int NCb = 0; int tm_inner = 0, tm_rows = 0;   // TMA box = tm_rows rows of tm_inner cells = one brick
     int MT = 0;                     // m-tiles of the tensor-core projections (0: FFMA2 loops), see sweep_brick.cuh
-    int nbuf = 1;                   // tile buffers of the sweep kernel (2: the next task's Q tile is prefetched)
     int nprob = 0, chunk = 0, nchunks = 0, nsrc = 0, nvol = 0;
     int G = 0, L = 0, NM = 0, ndir = 0, M = 0;
     int mode = 0, sweep_mode = 0, deterministic = 0;
@@ -65,11 +64,11 @@ struct PrepKey {
     unsigned long long inputs_version = 0;
     void* ws = nullptr;
     size_t total = 0;
-    int chunk = 0, B[3] = {0, 0, 0}, MT = 0, nbuf = 0, sweep_mode = 0, deterministic = 0, closure = 0, ctas_opt = 0;
+    int chunk = 0, B[3] = {0, 0, 0}, MT = 0, sweep_mode = 0, deterministic = 0, closure = 0, ctas_opt = 0;
     bool operator==(const PrepKey& k) const
     {
         return inputs_version == k.inputs_version && ws == k.ws && total == k.total && chunk == k.chunk && B[0] == k.B[0] &&
-               B[1] == k.B[1] && B[2] == k.B[2] && MT == k.MT && nbuf == k.nbuf && sweep_mode == k.sweep_mode && deterministic == k.deterministic &&
+               B[1] == k.B[1] && B[2] == k.B[2] && MT == k.MT && sweep_mode == k.sweep_mode && deterministic == k.deterministic &&
                closure == k.closure && ctas_opt == k.ctas_opt;
     }
 };
@@ -168,49 +167,28 @@ bool wants_mma(const doctors_solve_opts* o, int M)
     return pr == 2 || (pr == 0 && M > 16);
 }
 
-// Brick extents and the number of tile buffers (sweep_brick.cuh: NBUF).  The FMA-loop kernel runs double-buffered at two
-// CTAs per SM (the next task's Q tile in flight while this one is swept: config-4 slice 8.5 -> see profiles/r02_bench.md);
-// the tensor-core projections keep one tile.  `want_nbuf`: 0 automatic, 1 / 2 forced (doctors_solve_opts.tile_buffers).
-void auto_brick(int NM, int M, int nx, int ny, int nz, const int* req, bool mt, int want_nbuf, int B[3], int* nbuf_out)
+void auto_brick(int NM, int M, int nx, int ny, int nz, const int* req, bool mt, int B[3])
 {
-    auto fits = [&](int bx, int by, int bz, int nbuf, size_t limit) {
-        return brick_smem_layout(NM, bx, by, bz, M, mt ? projection_mtiles(NM, M, bx * by * bz) : 0, nbuf).total <= limit;
-    };
-    const size_t two_ctas = 113 * 1024, three_ctas = 74 * 1024, one_cta = 227 * 1024;
-    int nbuf = want_nbuf == 1 || want_nbuf == 2 ? want_nbuf : (mt ? 1 : 2);
-    if (mt) nbuf = 1;                                            // the padded-plane (mma) kernel exists single-buffered only
-    if (req && req[0] > 0 && req[1] > 0 && req[2] > 0) {
-        B[0] = req[0]; B[1] = req[1]; B[2] = req[2];
-        if (nbuf == 2 && !fits(B[0], B[1], B[2], 2, one_cta)) nbuf = 1;
-        *nbuf_out = nbuf;
-        return;
-    }
+    if (req && req[0] > 0 && req[1] > 0 && req[2] > 0) { B[0] = req[0]; B[1] = req[1]; B[2] = req[2]; return; }
     // cross section = the 32 lanes of a warp (8 x 4, reshaped for thin meshes); BX as long as shared memory allows
     B[1] = std::min(8, ny);
     B[2] = std::min(32 / B[1], nz);
     if (B[2] < 4 && B[1] < ny) B[1] = std::min(32 / B[2], ny);
-    const int cand[5] = {20, 16, 12, 8, 4};        // 20 x 8 x 4 = 640 cells = 2 per thread of a 320-thread CTA
-    auto pick = [&](int nb, size_t limit) {
-        for (int c = 0; c < 5; ++c) {
-            const int bx = std::min(cand[c], (nx + 3) / 4 * 4);
-            if (fits(bx, B[1], B[2], nb, limit)) return bx;
-        }
-        return 0;
+    const int cand[5] = {20, 16, 12, 8, 4};        // 20 x 8 x 4 = 640 cells = 2 per thread of a 320-thread CTA, 3 CTAs per SM
+    auto fits = [&](int bx, size_t limit) {
+        return brick_smem_layout(NM, bx, B[1], B[2], M, mt ? projection_mtiles(NM, M, bx * B[1] * B[2]) : 0).total <= limit;
     };
-    if (nbuf == 2) {
-        B[0] = pick(2, two_ctas);
-        if (B[0] >= 8 || (B[0] > 0 && nx <= 4)) { *nbuf_out = 2; return; }
-        nbuf = 1;                                                // the double-buffered tile does not fit a useful brick
+    for (int c = 0; c < 5; ++c) {
+        B[0] = std::min(cand[c], (nx + 3) / 4 * 4);
+        if (fits(B[0], 74 * 1024)) break;
     }
-    B[0] = pick(1, three_ctas);
     // many directions per octant (S16: 36 planes per tile): a brick shorter than 8 cells leaves 70 % of the wavefront's
     // lane-steps idle; two CTAs per SM with 8-cell bricks are faster (config 3: 2.86 against 3.47 ms per sweep)
-    if (B[0] < 8 && nx > 4) {
-        const int bx = pick(1, two_ctas);
-        if (bx > B[0]) B[0] = bx;
-    }
-    if (B[0] == 0) B[0] = 4;
-    *nbuf_out = 1;
+    if (B[0] < 8 && nx > 4)
+        for (int c = 0; c < 5; ++c) {
+            const int bx = std::min(cand[c], (nx + 3) / 4 * 4);
+            if (fits(bx, 113 * 1024)) { B[0] = bx; break; }
+        }
 }
 
 // Lay out the workspace.  chunk = problems solved together.
@@ -227,7 +205,7 @@ Plan make_plan(const doctors_problem* p, const doctors_solve_opts* o, int chunk)
     P.sweep_mode = o ? o->sweep_mode : 0;
     P.deterministic = o ? o->deterministic : 0;
     for (auto& s : p->sources) if (s.kind == 0) ++P.nvol;
-    auto_brick(P.NM, P.M, p->nx, p->ny, p->nz, o ? o->brick : nullptr, wants_mma(o, P.M), o ? o->tile_buffers : 0, P.B, &P.nbuf);
+    auto_brick(P.NM, P.M, p->nx, p->ny, p->nz, o ? o->brick : nullptr, wants_mma(o, P.M), P.B);
     P.gb[0] = (p->nx + P.B[0] - 1) / P.B[0];
     P.gb[1] = (p->ny + P.B[1] - 1) / P.B[1];
     P.gb[2] = (p->nz + P.B[2] - 1) / P.B[2];
@@ -240,8 +218,7 @@ Plan make_plan(const doctors_problem* p, const doctors_solve_opts* o, int chunk)
     P.tm_inner = P.NCb / P.tm_rows;
     P.ntasks = P.nbricks * 8 * P.chunk;
     P.MT = wants_mma(o, P.M) ? projection_mtiles(P.NM, P.M, P.NCb) : 0;
-    if (P.MT > 0) P.nbuf = 1;
-    P.smem = brick_smem_layout(P.NM, P.B[0], P.B[1], P.B[2], P.M, P.MT, P.nbuf).total;
+    P.smem = brick_smem_layout(P.NM, P.B[0], P.B[1], P.B[2], P.M, P.MT).total;
     { int dpw = (P.M + kMaxSweepWarps - 1) / kMaxSweepWarps; P.W = (P.M + dpw - 1) / dpw; }
 
     size_t off = 0;
@@ -588,8 +565,7 @@ int doctors_debug_schedule_dims(doctors_problem* p, const doctors_solve_opts* op
     if (level == 0) { dims[0] = p->nx; dims[1] = p->ny; dims[2] = p->nz; return DOCTORS_OK; }
     if (!p->has_xs || !p->has_quad) return fail(p, DOCTORS_BAD_STATE, "xs / quadrature not set (brick size depends on them)");
     int B[3];
-    int nbuf_unused = 1;
-    auto_brick((p->L + 1) * (p->L + 1), p->ndir / 8, p->nx, p->ny, p->nz, opts ? opts->brick : nullptr, wants_mma(opts, p->ndir / 8), opts ? opts->tile_buffers : 0, B, &nbuf_unused);
+    auto_brick((p->L + 1) * (p->L + 1), p->ndir / 8, p->nx, p->ny, p->nz, opts ? opts->brick : nullptr, wants_mma(opts, p->ndir / 8), B);
     if (level == 1) { for (int a = 0; a < 3; ++a) dims[a] = ((a == 0 ? p->nx : a == 1 ? p->ny : p->nz) + B[a] - 1) / B[a]; return DOCTORS_OK; }
     if (level == 2) { for (int a = 0; a < 3; ++a) dims[a] = B[a]; return DOCTORS_OK; }
     return fail(p, DOCTORS_INVALID_ARG, "level must be 0, 1 or 2");
@@ -717,41 +693,40 @@ int make_tensor_map(doctors_problem* p, CUtensorMap* tm, void* base, int rank, c
     return DOCTORS_OK;
 }
 
-template <int NM, bool FIX, int MT, int NBUF>
+template <int NM, bool FIX, int MT>
 cudaError_t launch_brick(const SweepLaunch& S, cudaStream_t st)
 {
-    k_sweep_brick<NM, FIX, MT, NBUF><<<S.grid, 32 * S.bp.W, S.smem, st>>>(S.tmQ, S.tmPhi, S.bp);
+    k_sweep_brick<NM, FIX, MT><<<S.grid, 32 * S.bp.W, S.smem, st>>>(S.tmQ, S.tmPhi, S.bp);
     return cudaGetLastError();
 }
 
-template <int NM, bool FIX, int MT, int NBUF>
+template <int NM, bool FIX, int MT>
 cudaError_t prep_brick(size_t smem, int threads, int* max_ctas)
 {
-    cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<NM, FIX, MT, NBUF>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+    cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<NM, FIX, MT>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(max_ctas, k_sweep_brick<NM, FIX, MT, NBUF>, threads, smem);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(max_ctas, k_sweep_brick<NM, FIX, MT>, threads, smem);
 }
 
-// NM in {1, 4, 9, 16}; MT > 0 only with NM = 16 (projection_mtiles) and only single-buffered; NBUF in {1, 2}
-#define DISPATCH_ONE(NMc, FIXc, MTc, NBc, EXPR) { constexpr int NM = NMc; constexpr bool FIX = FIXc; constexpr int MT = MTc; constexpr int NBUF = NBc; EXPR; }
-#define DISPATCH_NB(NMc, FIXc, NBv, EXPR) if ((NBv) == 2) DISPATCH_ONE(NMc, FIXc, 0, 2, EXPR) else DISPATCH_ONE(NMc, FIXc, 0, 1, EXPR)
-#define DISPATCH_NM(NMv, FIXc, MTv, NBv, EXPR)                                   \
+// NM in {1, 4, 9, 16}; MT > 0 only with NM = 16 (projection_mtiles)
+#define DISPATCH_ONE(NMc, FIXc, MTc, EXPR) { constexpr int NM = NMc; constexpr bool FIX = FIXc; constexpr int MT = MTc; EXPR; }
+#define DISPATCH_NM(NMv, FIXc, MTv, EXPR)                                        \
     switch (NMv) {                                                               \
-        case 1: DISPATCH_NB(1, FIXc, NBv, EXPR) break;                           \
-        case 4: DISPATCH_NB(4, FIXc, NBv, EXPR) break;                           \
-        case 9: DISPATCH_NB(9, FIXc, NBv, EXPR) break;                           \
+        case 1: DISPATCH_ONE(1, FIXc, 0, EXPR) break;                            \
+        case 4: DISPATCH_ONE(4, FIXc, 0, EXPR) break;                            \
+        case 9: DISPATCH_ONE(9, FIXc, 0, EXPR) break;                            \
         default:                                                                 \
             switch (MTv) {                                                       \
-                case 1: DISPATCH_ONE(16, FIXc, 1, 1, EXPR) break;                \
-                case 2: DISPATCH_ONE(16, FIXc, 2, 1, EXPR) break;                \
-                case 3: DISPATCH_ONE(16, FIXc, 3, 1, EXPR) break;                \
-                default: DISPATCH_NB(16, FIXc, NBv, EXPR) break;                 \
+                case 1: DISPATCH_ONE(16, FIXc, 1, EXPR) break;                   \
+                case 2: DISPATCH_ONE(16, FIXc, 2, EXPR) break;                   \
+                case 3: DISPATCH_ONE(16, FIXc, 3, EXPR) break;                   \
+                default: DISPATCH_ONE(16, FIXc, 0, EXPR) break;                  \
             }                                                                    \
             break;                                                               \
     }
-#define DISPATCH_NM_FIX(NMv, FIXv, MTv, NBv, EXPR)                               \
+#define DISPATCH_NM_FIX(NMv, FIXv, MTv, EXPR)                                    \
     do {                                                                         \
-        if (FIXv) { DISPATCH_NM(NMv, true, MTv, NBv, EXPR) } else { DISPATCH_NM(NMv, false, MTv, NBv, EXPR) } \
+        if (FIXv) { DISPATCH_NM(NMv, true, MTv, EXPR) } else { DISPATCH_NM(NMv, false, MTv, EXPR) } \
     } while (0)
 
 // TF32 rounding (round to nearest, ties away: what cvt.rna.tf32.f32 does) for the pre-split coefficient fragments
@@ -950,7 +925,7 @@ int prepare(doctors_problem* p, const doctors_solve_opts& o, const Plan& P)
         }
         int max_ctas = 0;
         cudaError_t e = cudaSuccess;
-        DISPATCH_NM_FIX(NM, o.closure == 1, P.MT, P.nbuf, e = (prep_brick<NM, FIX, MT, NBUF>(P.smem, 32 * P.W, &max_ctas)));
+        DISPATCH_NM_FIX(NM, o.closure == 1, P.MT, e = (prep_brick<NM, FIX, MT>(P.smem, 32 * P.W, &max_ctas)));
         if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "sweep kernel setup failed: %s (smem %zu)", cudaGetErrorString(e), P.smem);
         if (max_ctas < 1) return fail(p, DOCTORS_CUDA, "sweep kernel does not fit an SM (smem %zu)", P.smem);
         ctas_per_sm = o.ctas_per_sm > 0 ? std::min(o.ctas_per_sm, max_ctas) : max_ctas;
@@ -969,7 +944,6 @@ int prepare(doctors_problem* p, const doctors_solve_opts& o, const Plan& P)
         bp.flags = at<unsigned>(p, P.o_flags);
         bp.faceX = at<double>(p, P.o_fx); bp.faceY = at<double>(p, P.o_fy); bp.faceZ = at<double>(p, P.o_fz);
         bp.dbg_plane = nullptr;
-        bp.nbuf = P.nbuf;
         bp.bulk_faces = (P.face_x_n % 2 == 0 && P.face_y_n % 2 == 0 && P.face_z_n % 2 == 0) ? 1 : 0;
         bp.state = at<ProbState>(p, P.o_state);
         bp.leak = at<double>(p, P.o_leak);
@@ -1007,7 +981,6 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
     const bool adaptive_window = o.check_window <= 0;   // first host read where the previous group stopped, then every sweep
     if (o.check_window <= 0) o.check_window = 12;
     if (o.closure != 0 && o.closure != 1) return fail(p, DOCTORS_INVALID_ARG, "closure must be 0 or 1");
-    if (o.tile_buffers < 0 || o.tile_buffers > 2) return fail(p, DOCTORS_INVALID_ARG, "tile_buffers must be 0 (automatic), 1 or 2");
     if (o.sweep_mode < 0 || o.sweep_mode > 1) return fail(p, DOCTORS_INVALID_ARG, "sweep_mode must be 0 or 1");
     if (o.brick[0] > 0 && (o.brick[0] % 4 != 0 || o.brick[0] > 64 || o.brick[1] <= 0 || o.brick[2] <= 0 || o.brick[1] * o.brick[2] > 32))
         return fail(p, DOCTORS_INVALID_ARG, "brick: brick[0] a multiple of 4 (<= 64), brick[1] * brick[2] <= 32 (the lanes of a warp)");
@@ -1032,7 +1005,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
 
     PrepKey key;
     key.inputs_version = p->inputs_version; key.ws = p->ws; key.total = P.total; key.chunk = P.chunk;
-    key.B[0] = P.B[0]; key.B[1] = P.B[1]; key.B[2] = P.B[2]; key.MT = P.MT; key.nbuf = P.nbuf; key.sweep_mode = P.sweep_mode;
+    key.B[0] = P.B[0]; key.B[1] = P.B[1]; key.B[2] = P.B[2]; key.MT = P.MT; key.sweep_mode = P.sweep_mode;
     key.deterministic = P.deterministic; key.closure = o.closure; key.ctas_opt = o.ctas_per_sm;
     if (!p->prepared || !(p->prep_key == key)) {
         p->prepared = false;
@@ -1169,7 +1142,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
                             // problems done (k_group_begin), so their tasks are skipped
                             SL.bp.ntasks = oct_begin[l + 1] - oct_begin[l];
                             cudaError_t e;
-                            DISPATCH_NM_FIX(NM, o.closure == 1, P.MT, P.nbuf, e = (launch_brick<NM, FIX, MT, NBUF>(SL, st)));
+                            DISPATCH_NM_FIX(NM, o.closure == 1, P.MT, e = (launch_brick<NM, FIX, MT>(SL, st)));
                             if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "sweep launch failed: %s", cudaGetErrorString(e));
                             ++sweep_launches; ++kernel_launches;
                         }
@@ -1247,7 +1220,6 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         info->brick[0] = P.B[0]; info->brick[1] = P.B[1]; info->brick[2] = P.B[2];
         info->ctas_per_sm = ctas_per_sm;
         info->projection_mtiles = P.sweep_mode == 0 ? P.MT : 0;
-        info->tile_buffers = P.sweep_mode == 0 ? P.nbuf : 0;
         info->sweep_kernel = o.sweep_mode == 1 ? 1 : 0;
         info->timed_sweeps = (unsigned long long)(sweep_ev.size() / 2);
         info->pl_exceeds_quadrature = p->pl_inexact;
@@ -1284,7 +1256,7 @@ extern "C" int doctors_debug_device_brick_steps(doctors_problem* p, int bx, int 
         return fail(p, DOCTORS_INVALID_ARG, "brick: bx a multiple of 4 (<= 64), by * bz <= 32");
     CK(cudaSetDevice(p->device));
     const int NC = bx * by * bz;
-    const size_t smem = brick_smem_layout(1, bx, by, bz, 1, 0, 1).total;
+    const size_t smem = brick_smem_layout(1, bx, by, bz, 1, 0).total;
     // scratch: Q, phi (float), sigt (double), faces (double), table blobs, control
     struct Scratch { float* Q; float* phi; double* sig; double* face; unsigned char* tab; uint2* task;
                      unsigned* flags; Control* ctl; ProbState* st; double* leak; int* planes; } S;
@@ -1325,7 +1297,7 @@ extern "C" int doctors_debug_device_brick_steps(doctors_problem* p, int bx, int 
     }
     BrickParams& bp = SL.bp;
     std::memset(&bp, 0, sizeof bp);
-    bp.tm_rows = rows; bp.nprob = 1; bp.nbuf = 1;
+    bp.tm_rows = rows; bp.nprob = 1;
     bp.nx = bx; bp.ny = by; bp.nz = bz; bp.BX = bx; bp.BY = by; bp.BZ = bz; bp.gbx = bp.gby = bp.gbz = 1;
     bp.M = 1; bp.W = 1; bp.g = 0; bp.Gs = 1; bp.epoch = 1; bp.task_begin = 0; bp.ntasks = 1; bp.counter_slot = 0;
     bp.NCb = NC; bp.cells_p = NC; bp.Q = S.Q; bp.phi = S.phi; bp.sigt = S.sig; bp.octtab = S.tab;
@@ -1333,9 +1305,9 @@ extern "C" int doctors_debug_device_brick_steps(doctors_problem* p, int bx, int 
     bp.faceX = S.face; bp.faceY = S.face + size_t(by) * bz; bp.faceZ = bp.faceY + size_t(bx) * bz;
     bp.state = S.st; bp.leak = S.leak;
     bp.dbg_plane = S.planes;
-    cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<1, false, 0, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+    cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<1, false, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
     if (e == cudaSuccess) {
-        k_sweep_brick<1, false, 0, 1, true><<<1, 32, smem, p->stream>>>(SL.tmQ, SL.tmPhi, bp);
+        k_sweep_brick<1, false, 0, true><<<1, 32, smem, p->stream>>>(SL.tmQ, SL.tmPhi, bp);
         e = cudaGetLastError();
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);

@@ -61,7 +61,6 @@ struct BrickParams {
     double* faceZ;               // [prob][8][gbx*gby][M][BY][BX]
     const ProbState* state;
     double* leak;                // [prob]
-    int nbuf;                    // tile buffers in shared memory (1 or 2), must match the kernel's NBUF
     int bulk_faces;              // 1: all three face blocks are multiples of 16 bytes -> moved by bulk async copies (TMA unit)
     int* dbg_plane;              // debug hook: NULL, or [BX*BY*BZ] receives the step at which each cell of a full brick is visited
 };
@@ -99,32 +98,26 @@ __host__ __device__ inline int plane_pitch(int NC, int MT)
 }
 
 struct BrickSmem {
-    size_t q, qstride, sig, fx, fy, fz, tab, tabstride, done, misc, total;
+    size_t q, sig, psi, fx, fy, fz, tab, done, misc, total;
 };
 
-// nbuf = 1: one tile, loaded at the start of its task (three CTAs per SM on config 4's shapes).
-// nbuf = 2: two tiles and two table blobs: the Q tile of the NEXT task is in flight while the current one is swept
-//           (two CTAs per SM); see the kernel's header comment.
-__host__ __device__ inline BrickSmem brick_smem_layout(int NM, int BX, int BY, int BZ, int M, int MT, int nbuf)
+__host__ __device__ inline BrickSmem brick_smem_layout(int NM, int BX, int BY, int BZ, int M, int MT)
 {
     BrickSmem s;
     size_t NC = size_t(BX) * BY * BZ, o = 0;
-    s.misc = o;  o = align_up(o + 128, 128);   // mbarriers, task slots, reduction scratch
+    s.misc = o;  o = align_up(o + 128, 128);   // mbarrier, task slots, reduction scratch
     // front pad: a wavefront lane that has not reached its x range yet loads from its running address, up to
     // (BY + BZ - 2) steps of BY cells (8 bytes each for sigma_t) BEFORE its row — that must still be this CTA's memory
     o = align_up(o + size_t(8) * BY * (BY + BZ - 2), 128);
     // one tile of max(NM, M) planes holds, in turn, Q_lm (bulk loads), psi_n (in place, per cell) and the
     // phi_lm contribution (in place again, bulk reduce-add source)
-    s.q = o;
-    s.qstride = align_up(size_t(NM > M ? NM : M) * plane_pitch(int(NC), MT) * 4, 128);
-    o += s.qstride * size_t(nbuf);
+    s.q = o;     o = align_up(o + size_t(NM > M ? NM : M) * plane_pitch(int(NC), MT) * 4, 128);
     s.sig = o;   o = align_up(o + NC * 8, 128);
+    s.psi = s.q;
     s.fx = o;    o = align_up(o + size_t(M) * BY * BZ * 8, 8);      // fx, fy, fz contiguous (one load loop)
     s.fy = o;    o = align_up(o + size_t(M) * BX * BZ * 8, 8);
     s.fz = o;    o = align_up(o + size_t(M) * BX * BY * 8, 16);
-    s.tab = o;
-    s.tabstride = align_up(octtab_layout(NM, M, MT).total, 16);
-    o += s.tabstride * size_t(nbuf);
+    s.tab = o;   o = align_up(o + octtab_layout(NM, M, MT).total, 16);
     s.done = o;  o = align_up(o + 256, 16);      // "problem has stopped" bytes of the launch (task prob index is 8 bits)
     o = align_up(o + 128 + size_t(8) * BY * (BY + BZ - 2), 16);   // tail pad: lanes past their x range (sx < 0: before it) overshoot by the same amount
     s.total = o;
@@ -295,129 +288,82 @@ __device__ __noinline__ void project_directions_to_moments_mma(uint32_t tile, ui
     }
 }
 
-// NBUF = 2 (software pipeline, two CTAs per SM): the Q tile of the NEXT task is loaded into the second tile buffer while
-// the current task is swept, and sigma_t / the octant tables of the next task follow as soon as the wavefront has
-// released them.  Measured on config 4 (profiles/r02_sweep_ncu.md): the data movement of a sweep alone takes 5.3 ms per
-// 2-problem launch (DRAM-bound), the arithmetic alone 4.4 ms, the single-buffered kernel 8.5 ms — a CTA that loads does
-// not compute, and three CTAs per SM do not cover each other.  NBUF = 1: one tile, three CTAs per SM (the tensor-core
-// projections and shapes whose double-buffered tile does not fit).
-template <int NM, bool FIX, int MT, int NBUF, bool DBG = false>
-__global__ void __launch_bounds__(32 * kMaxSweepWarps, NBUF == 2 ? 2 : 3)
+template <int NM, bool FIX, int MT, bool DBG = false>
+__global__ void __launch_bounds__(32 * kMaxSweepWarps, 3)
 k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmPhi, const BrickParams P)
 {
     static_assert(MT == 0 || NM == 16, "tensor-core projections are written for P3 (16 moments)");
     static_assert(NM <= 16, "one tile-warp lane per moment plane, lanes 16 / 17 for sigma_t and the tables");
-    static_assert(NBUF == 1 || NBUF == 2, "one or two tile buffers");
     if (__ldcg(&P.ctl->all_done)) return;                              // every problem of the chunk has stopped (a6): nothing to sweep
     extern __shared__ __align__(128) unsigned char smem[];
     const int BX = P.BX, BY = P.BY, BZ = P.BZ, M = P.M;
     const int NC = BX * BY * BZ;
     const int NCP = plane_pitch(NC, MT);                              // plane pitch of the tile (floats)
-    const BrickSmem L = brick_smem_layout(NM, BX, BY, BZ, M, MT, NBUF);
+    const BrickSmem L = brick_smem_layout(NM, BX, BY, BZ, M, MT);
     const OctTab T = octtab_layout(NM, M, MT);
+    float* sQ = reinterpret_cast<float*>(smem + L.q);
     double* sSig = reinterpret_cast<double*>(smem + L.sig);
+    float* sPsi = reinterpret_cast<float*>(smem + L.psi);
     double* sFx = reinterpret_cast<double*>(smem + L.fx);
     double* sFy = reinterpret_cast<double*>(smem + L.fy);
     double* sFz = reinterpret_cast<double*>(smem + L.fz);
-    // mbarriers: Q tile of buffer 0 / 1, sigma_t + tables, faces; then the task ring and the leakage scratch
+    double* sDir = reinterpret_cast<double*>(smem + L.tab + T.dir);  // [M][4]
+    float4* sLk = reinterpret_cast<float4*>(smem + L.tab + T.lk);
+    float* sM = reinterpret_cast<float*>(smem + L.tab + T.t0);      // MT = 0: [M][pitch];  MT >= 1: A fragments (float4 per lane)
+    float* sD = reinterpret_cast<float*>(smem + L.tab + T.t2);
     uint64_t* sBar = reinterpret_cast<uint64_t*>(smem + L.misc);
-    int* sTask = reinterpret_cast<int*>(smem + L.misc + 32);        // [3]
-    uint2* sDesc = reinterpret_cast<uint2*>(smem + L.misc + 48);   // [3]
-    float* sRed = reinterpret_cast<float*>(smem + L.misc + 80);     // kMaxSweepWarps floats
+    int* sTask = reinterpret_cast<int*>(smem + L.misc + 8);
+    float* sRed = reinterpret_cast<float*>(smem + L.misc + 64);     // kMaxSweepWarps floats
 
     const int tid = threadIdx.x, nthr = blockDim.x;
     const int lane = tid & 31, warp = tid >> 5;
-    const uint32_t barQ = smem_u32(sBar);                            // + 8 * buffer
-    const uint32_t barS = barQ + 16, barF = barQ + 24;
+    const uint32_t bar = smem_u32(sBar);
     int jp, kp;
     lane_cross_section(lane, BY, jp, kp);
 
-    if (tid == 0) { mbar_init(barQ, 1); mbar_init(barQ + 8, 1); mbar_init(barS, 1); mbar_init(barF, P.bulk_faces ? 3 : 1); fence_mbar_init(); }
+    const uint32_t barF = bar + 32;                                  // faces (bulk copies) complete here
+    if (tid == 0) { mbar_init(bar, 1); mbar_init(barF, P.bulk_faces ? 3 : 1); fence_mbar_init(); }
+    uint32_t parity = 0;
     const int faceXn = M * BY * BZ, faceYn = M * BX * BZ, faceZn = M * BX * BY;
     const int nbricks = P.gbx * P.gby * P.gbz;
+    int last_oct = -1;
 
     // Roles inside the CTA (all of them also sweep):
-    //   tile warp   lane 0 (lanes 0..NM-1 with padded planes): tensor / bulk load of Q_lm, bulk reduce-add of the phi_lm
-    //               contribution (same lane = same bulk group, so the lane can wait for "read done"); lanes 16 / 17:
-    //               sigma_t and the octant's table blob
+    //   tile warp   lanes 0..NM-1 own one moment plane each: bulk load of Q_lm at the start of a task, bulk reduce-add of
+    //               the phi_lm contribution at its end (same lane = same bulk group, so the lane can wait for "read done")
     //   pollers     warp 0, lanes 0..2: wait for the upwind brick in x / y / z and issue that face's bulk load themselves
-    //   prefetcher  one thread keeps the task ring two tasks ahead (id from the atomic counter, then its descriptor; tasks of
-    //               problems that have stopped are dropped here).  Holding unstarted tasks cannot deadlock: a CTA's held
-    //               tasks have higher indices than its running one, so the lowest unfinished task of the grid is always running.
-    //   publisher   last lane of the last warp: bulk-stores the outflow faces and releases the brick's flag after the
-    //               end-of-task barrier
+    //   prefetcher  one thread fetches the NEXT task (id from the atomic counter, then its descriptor) into shared memory
+    //               while the current one runs: two dependent global round trips off the critical path.
+    //               Holding one unstarted task cannot deadlock: a CTA's held task has a higher index than its running one,
+    //               so the lowest unfinished task of the whole grid is always running.
+    //   publisher   last lane of the last warp: bulk-stores the outflow faces, and at the next loop top waits for them and
+    //               releases the brick's flag AFTER arriving at the block barrier (split barrier: nobody waits for it)
     const int nwarps = nthr >> 5;
     const int tileWarp = nwarps > 1 ? 1 : 0;
     const int pfThread = nwarps > 2 ? 64 : 32 * tileWarp + 8;
     const int pubWarp = nwarps - 1;
+    uint2* sDesc = reinterpret_cast<uint2*>(smem + L.misc + 16);   // [2]
     unsigned char* sDoneP = smem + L.done;                        // [nprob]: fixed for the whole launch (k_check runs between launches)
     for (int q = tid; q < P.nprob; q += nthr) sDoneP[q] = (unsigned char)(__ldcg(&P.state[q].done) != 0);
-    __syncthreads();                                             // stop flags, mbarriers
     auto fetch_task = [&](int sl) {
-        int id;
-        uint2 d;
-        do {                                                     // skip the tasks of problems that have stopped (a6)
-            id = int(atomicAdd(&P.ctl->counters[P.counter_slot], 1u));
-            d = make_uint2(0u, 0u);
-            if (id < P.ntasks) d = P.tasks[P.task_begin + id];
-        } while (id < P.ntasks && sDoneP[d.x & 0xff]);
+        const int id = int(atomicAdd(&P.ctl->counters[P.counter_slot], 1u));
+        uint2 d = make_uint2(0u, 0u);
+        if (id < P.ntasks) d = P.tasks[P.task_begin + id];
         sDesc[sl] = d; sTask[sl] = id;
     };
-    // Q_lm tile of task d -> tile buffer b (tensor copy; one bulk copy per plane where the planes are padded)
-    auto issue_q = [&](const uint2 d, const int b) {
-        const int prob_ = d.x & 0xff;
-        const int brick_ = int(d.y & 0x3ff) + P.gbx * (int((d.y >> 10) & 0x3ff) + P.gby * int((d.y >> 20) & 0x3ff));
-        float* dst = reinterpret_cast<float*>(smem + L.q + size_t(b) * L.qstride);
-        if constexpr (MT == 0) {
-            // dense tile [NM][brick]: ONE tensor copy (4-D box {row, rows of the brick, moments, problem}); issuing a bulk
-            // operation costs ~200 cycles of the issuing warp, so one per moment plane is only used where the planes
-            // are padded in shared memory (tensor-core projections)
-            if (lane == 0) {
-                bulk_wait_read0();                               // the reduce-add that last used this buffer has read it
-                mbar_expect_tx(barQ + 8u * b, uint32_t(NM * NC * 4));
-                tma_load_4d(smem_u32(dst), &tmQ, barQ + 8u * b, 0, P.tm_rows * brick_, 0, prob_);
-            }
-        } else {
-            if (lane == 0) mbar_expect_tx(barQ + 8u * b, uint32_t(NM * NC * 4));
-            if (lane < NM) {
-                bulk_wait_read0();                               // this lane's reduce-add has read its plane
-                const float* gq = P.Q + (size_t)prob_ * NM * P.cells_p + (size_t)brick_ * P.NCb;
-                bulk_load(smem_u32(dst + lane * NCP), gq + (size_t)lane * P.cells_p, uint32_t(NC * 4), barQ + 8u * b);
-            }
-        }
-    };
-    // sigma_t of task d's brick and, if `tab`, the table blob of its octant -> table buffer tb
-    auto issue_s = [&](const uint2 d, const int tb, const bool tab) {
-        const int oct_ = (d.x >> 8) & 7;
-        const int brick_ = int(d.y & 0x3ff) + P.gbx * (int((d.y >> 10) & 0x3ff) + P.gby * int((d.y >> 20) & 0x3ff));
-        if (lane == 16) {
-            mbar_expect_tx(barS, uint32_t(NC * 8 + (tab ? T.total : 0)));
-            bulk_load(smem_u32(sSig), P.sigt + (size_t)brick_ * P.NCb, uint32_t(NC * 8), barS);
-        }
-        if (tab && lane == 17) bulk_load(smem_u32(smem + L.tab + size_t(tb) * L.tabstride), P.octtab + (size_t)oct_ * T.total, uint32_t(T.total), barS);
-    };
-    if (tid == 0) { fetch_task(0); fetch_task(1); }
-    __syncthreads();
-    int s0 = 0;                                                  // ring slot of the current task
-    int buf = 0, tbuf = 0;                                       // tile / table buffer of the current task
-    int tabOct0 = -1, tabOct1 = -1;                              // octant whose tables sit in table buffer 0 / 1
-    uint32_t parQ = 0, parS = 0, parF = 0;                       // parities to wait for (bit b of parQ: tile buffer b)
-    if (NBUF == 2 && sTask[0] < P.ntasks && warp == tileWarp) {  // prologue of the pipeline: the first task's loads
-        issue_q(sDesc[0], 0);
-        issue_s(sDesc[0], 0, true);
-    }
-    if (NBUF == 2) tabOct0 = (sDesc[0].x >> 8) & 7;
+    if (tid == 0) fetch_task(0);
+    __syncthreads();                                             // mbarriers, first task, stop flags
+    int slot = 0;
     // ONE block barrier ends a task (after phase 2): behind it nobody reads the tile, the tables, the faces or the task
     // slot of that task any more, so the next task starts without a barrier of its own.
     while (true) {
-        const int t = sTask[s0];
+        const int t = sTask[slot];
         if (t >= P.ntasks) break;
-        const uint2 td = sDesc[s0];
-        const int s1 = s0 == 2 ? 0 : s0 + 1, s2 = s1 == 2 ? 0 : s1 + 1;
-        const bool have_next = sTask[s1] < P.ntasks;
-        const uint2 td1 = sDesc[s1];
-        if (tid == pfThread) fetch_task(s2);                     // slot s2 held the previous task: everybody is past it (end-of-task barrier)
-        s0 = s1;
+        const uint2 td = sDesc[slot];
+        const int prob_done = sDoneP[td.x & 0xff];
+        if (tid == pfThread) fetch_task(slot ^ 1);
+        slot ^= 1;
+        if (prob_done) { __syncthreads(); continue; }            // this problem has stopped (a6); the barrier orders the task slots
         const int prob = td.x & 0xff, oct = (td.x >> 8) & 7;
         const int bi = td.y & 0x3ff, bj = (td.y >> 10) & 0x3ff, bk = (td.y >> 20) & 0x3ff;
 
@@ -437,19 +383,28 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         double* gFy = P.faceY + (po * (P.gbx * P.gbz) + bi + P.gbx * bk) * (size_t)faceYn;
         double* gFz = P.faceZ + (po * (P.gbx * P.gby) + bi + P.gbx * bj) * (size_t)faceZn;
 
-        if (NBUF == 1) {
-            // one tile: its loads start here (nobody reads the old tile or tables any more: end-of-task barrier)
-            const bool tab = oct != tabOct0;
-            if (warp == tileWarp) { issue_q(td, 0); issue_s(td, 0, tab); }
-            tabOct0 = oct;
+        // tile, sigma_t and (when the octant changes) the octant's table blob: bulk async copies, one mbarrier.
+        // Directions of an octant are contiguous (n = oct*M + m); nobody reads the old tables any more (loop-top barrier).
+        if (warp == tileWarp) {
+            const bool tab = oct != last_oct;
+            if (lane == 0) mbar_expect_tx(bar, uint32_t(NM * NC * 4 + NC * 8 + (tab ? T.total : 0)));
+            const float* gq = P.Q + (size_t)prob * NM * P.cells_p + (size_t)brick * P.NCb;
+            if constexpr (MT == 0) {
+                // dense tile [NM][brick]: ONE tensor copy (4-D box {row, rows of the brick, moments, problem}); issuing a bulk
+                // operation costs ~200 cycles of the issuing warp, so one per moment plane is only used where the planes
+                // are padded in shared memory (tensor-core projections)
+                if (lane == 0) {
+                    bulk_wait_read0();                           // the reduce-add of the previous task has read the tile
+                    tma_load_4d(smem_u32(sQ), &tmQ, bar, 0, P.tm_rows * brick, 0, prob);
+                }
+            } else if (lane < NM) {
+                bulk_wait_read0();                               // this lane's reduce-add of the previous task has read its plane
+                bulk_load(smem_u32(sQ + lane * NCP), gq + (size_t)lane * P.cells_p, uint32_t(NC * 4), bar);
+            }
+            if (lane == 16) bulk_load(smem_u32(sSig), P.sigt + (size_t)brick * P.NCb, uint32_t(NC * 8), bar);
+            if (tab && lane == 17) bulk_load(smem_u32(smem + L.tab), P.octtab + (size_t)oct * T.total, uint32_t(T.total), bar);
         }
-        float* sQ = reinterpret_cast<float*>(smem + L.q + size_t(buf) * L.qstride);
-        float* sPsi = sQ;
-        const unsigned char* tabp = smem + L.tab + size_t(tbuf) * L.tabstride;
-        const double* sDir = reinterpret_cast<const double*>(tabp + T.dir);  // [M][4]
-        const float4* sLk = reinterpret_cast<const float4*>(tabp + T.lk);
-        const float* sM = reinterpret_cast<const float*>(tabp + T.t0);      // MT = 0: [M][pitch];  MT >= 1: A fragments (float4 per lane)
-        const float* sD = reinterpret_cast<const float*>(tabp + T.t2);
+        last_oct = oct;
         // wait for the upwind bricks of this (problem, octant): one warp-0 lane per upwind flag
         if (P.bulk_faces) {
             if (warp == 0 && lane < 3) {
@@ -503,10 +458,8 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
                 sFx[e] = u ? __ldcg(src) : 0.0;
             }
         }
-        mbar_wait(barS, parS);                                   // sigma_t and the tables of this task
-        parS ^= 1u;
-        mbar_wait(barQ + 8u * buf, (parQ >> buf) & 1u);          // its Q tile
-        parQ ^= 1u << buf;
+        mbar_wait(bar, parity);
+        parity ^= 1u;
 
         // ---- phase 0: q_n = sum_lm Mtab[n][lm] Q_lm for every cell of the brick (a5) ----
         if constexpr (MT >= 1) {
@@ -546,12 +499,8 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
                 }
             }
         }
-        // pipeline: the NEXT task's Q tile goes into the other buffer now (the reduce-add that used it was issued a whole
-        // task ago), and has the wavefront and phase 2 of this task to arrive
-        if (NBUF == 2 && have_next && warp == tileWarp) issue_q(td1, buf ^ 1);
         if (P.bulk_faces) {
-            mbar_wait(barF, parF);
-            parF ^= 1u;
+            mbar_wait(barF, parity ^ 1u);                         // same phase sequence as `bar` (flipped above)
         } else {
 #pragma unroll
             for (int k = 0; k < kFaceRegs; ++k) {
@@ -612,16 +561,6 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         }
         if (P.bulk_faces) fence_proxy_async_smem();              // lanes' face writes -> visible to the async proxy
         __syncthreads();
-        // pipeline: sigma_t is free now, and the table buffer this task does not use; the next task's copies start
-        int tbuf_next = tbuf;
-        if (NBUF == 2 && have_next) {
-            const int oct1 = (td1.x >> 8) & 7;
-            const bool same = oct1 == (tbuf ? tabOct1 : tabOct0);
-            if (!same) tbuf_next = tbuf ^ 1;
-            const bool tab = !same && oct1 != (tbuf_next ? tabOct1 : tabOct0);
-            if (warp == tileWarp) issue_s(td1, tbuf_next, tab);
-            if (tbuf_next) tabOct1 = oct1; else tabOct0 = oct1;
-        }
         // ---- outflow faces to the downwind bricks: bulk async stores issued by the publisher (last lane of the last warp) ----
         if (P.bulk_faces && warp == pubWarp && lane == 31) {
             if (dnx) bulk_store(gFx, smem_u32(sFx), uint32_t(8 * faceXn));
@@ -722,7 +661,6 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
             fence_proxy_async_global();
             st_release_u32(flag_base + brick, P.epoch);
         }
-        if (NBUF == 2) { buf ^= 1; tbuf = tbuf_next; }
     }
     if (warp == tileWarp) bulk_wait0();
 }

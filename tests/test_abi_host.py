@@ -45,9 +45,9 @@ def test_struct_layouts_match_the_library(pkg):
     L.doctors_abi_sizes(sizes)
     from paper_1910_11335_b200 import binding
     assert tuple(sizes) == (ctypes.sizeof(binding.CSource), ctypes.sizeof(binding.CSolveOpts), ctypes.sizeof(binding.CSolveInfo))
-    assert [f[0] for f in binding.CSolveOpts._fields_][-3:] == ["check_window", "projection", "tile_buffers"]
-    assert [f[0] for f in binding.CSolveInfo._fields_][-5:] == ["sweep_kernel", "projection_mtiles", "tile_buffers",
-                                                                "timed_sweeps", "pl_exceeds_quadrature"]
+    assert [f[0] for f in binding.CSolveOpts._fields_][-2:] == ["check_window", "projection"]
+    assert [f[0] for f in binding.CSolveInfo._fields_][-4:] == ["sweep_kernel", "projection_mtiles", "timed_sweeps",
+                                                                "pl_exceeds_quadrature"]
 
 
 def test_version_and_no_device_error(pkg):
