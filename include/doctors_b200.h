@@ -194,7 +194,9 @@ int doctors_debug_get_schedule(doctors_problem* p, const doctors_solve_opts* opt
 /* Device-side check of the in-brick wavefront (level 2): runs the product sweep kernel on one full
  * bx x by x bz brick for `octant` and returns, per cell (local index li + bx*(lj + by*lk)), the step at
  * which the kernel updated it.  By Eq. (8) that step must equal the cell's sub-sweep
- * index i'+j'+k' in the octant's sweep-space coordinates.  Needs a CUDA device. */
+ * index i'+j'+k' in the octant's sweep-space coordinates.  The same launch bounds-checks every shared-memory address of the
+ * wavefront loop, idle lanes included (they load from their running addresses): an address outside the CTA's allocation makes
+ * the call return DOCTORS_CUDA (compute-sanitizer is closed on this pool; this is the repo's own check).  Needs a CUDA device. */
 int doctors_debug_device_brick_steps(doctors_problem* p, int bx, int by, int bz, int octant, int32_t* step_of_cell);
 /* P(S) of Eq. (9) as the library evaluates it. */
 long long doctors_wavefront_size(int nx, int ny, int nz, int S);

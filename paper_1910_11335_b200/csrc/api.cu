@@ -1263,13 +1263,13 @@ extern "C" int doctors_debug_device_brick_steps(doctors_problem* p, int bx, int 
     const size_t nface = size_t(by) * bz + size_t(bx) * bz + size_t(bx) * by;
     const OctTab T = octtab_layout(1, 1, 0);
     char* base = nullptr;
-    const size_t bytes = 8192 + size_t(NC) * (4 + 4 + 8 + 4) + nface * 8 * 2 + 8 * T.total;
+    const size_t bytes = 8192 + size_t(NC) * (4 + 4 + 8 + 4) + 256 + nface * 8 * 2 + 8 * T.total;
     CK(cudaMalloc(&base, bytes));
     CK(cudaMemset(base, 0, bytes));
     size_t off = 0;
     auto take = [&](size_t n) { char* r = base + off; off = align_up(off + n, 256); return r; };
     S.Q = (float*)take(size_t(NC) * 4); S.phi = (float*)take(size_t(NC) * 4); S.sig = (double*)take(size_t(NC) * 8);
-    S.planes = (int*)take(size_t(NC) * 4); S.face = (double*)take(nface * 8);
+    S.planes = (int*)take(size_t(NC) * 4 + 4); S.face = (double*)take(nface * 8);
     S.tab = (unsigned char*)take(8 * T.total); S.task = (uint2*)take(16);
     S.flags = (unsigned*)take(64); S.ctl = (Control*)take(sizeof(Control)); S.st = (ProbState*)take(sizeof(ProbState)); S.leak = (double*)take(8);
     if (off > bytes) { cudaFree(base); return fail(p, DOCTORS_ALLOC, "debug scratch too small"); }
@@ -1311,9 +1311,12 @@ extern "C" int doctors_debug_device_brick_steps(doctors_problem* p, int bx, int 
         e = cudaGetLastError();
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
-    std::vector<int32_t> stored(size_t(NC), -1);
-    if (e == cudaSuccess) e = cudaMemcpy(stored.data(), S.planes, size_t(NC) * 4, cudaMemcpyDeviceToHost);
+    std::vector<int32_t> stored(size_t(NC) + 1, -1);
+    if (e == cudaSuccess) e = cudaMemcpy(stored.data(), S.planes, size_t(NC) * 4 + 4, cudaMemcpyDeviceToHost);
     cudaFree(base);
+    if (e == cudaSuccess && stored[size_t(NC)] != 0)
+        return fail(p, DOCTORS_CUDA, "wavefront loop: %d shared-memory addresses outside the CTA's allocation (brick %d x %d x %d, octant %d)",
+                    int(stored[size_t(NC)]), bx, by, bz, octant);
     for (int lk = 0; lk < bz; ++lk)                             // storage order inside a brick (y fastest) -> documented order
         for (int lj = 0; lj < by; ++lj)
             for (int li = 0; li < bx; ++li) step_of_cell[li + bx * (lj + by * lk)] = stored[size_t(lj + by * (li + bx * lk))];

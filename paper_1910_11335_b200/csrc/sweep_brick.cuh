@@ -62,7 +62,8 @@ struct BrickParams {
     const ProbState* state;
     double* leak;                // [prob]
     int bulk_faces;              // 1: all three face blocks are multiples of 16 bytes -> moved by bulk async copies (TMA unit)
-    int* dbg_plane;              // debug hook: NULL, or [BX*BY*BZ] receives the step at which each cell of a full brick is visited
+    int* dbg_plane;              // debug hook: NULL, or [BX*BY*BZ + 1]: the step at which each cell of a full brick is visited,
+                                 // then the count of out-of-allocation shared-memory addresses of the wavefront loop
 };
 
 __host__ __device__ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -554,7 +555,15 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
                 sts_f64_if(act && ly, py, oy);
                 sts_f64_if(act && lz, pz, oz);
                 if (act) ax = ox;
-                if (DBG && act) P.dbg_plane[(pq - smem_u32(sPsi)) / 4u - uint32_t(n * NCP)] = nsteps - s;   // indexed by the storage order (y fastest)
+                if (DBG) {
+                    // debug instantiation (doctors_debug_device_brick_steps): the step at which each cell is visited, and a
+                    // bounds check of EVERY shared-memory address of the step, idle lanes included (they load from their
+                    // running addresses, see above): slot NC of dbg_plane counts addresses outside this CTA's allocation
+                    if (act) P.dbg_plane[(pq - smem_u32(sPsi)) / 4u - uint32_t(n * NCP)] = nsteps - s;   // indexed by the storage order (y fastest)
+                    const uint32_t lo = smem_u32(smem), hi = lo + uint32_t(L.total);
+                    const bool bad = pq < lo || pq + 4u > hi || ps < lo || ps + 8u > hi || py < lo || py + 8u > hi || pz < lo || pz + 8u > hi;
+                    if (bad) atomicAdd(P.dbg_plane + NC, 1);
+                }
                 ++ip; pq += d4; ps += d8; py += d8f; pz += d8f;
             }
             if (lane_ok) *fxp = ax;

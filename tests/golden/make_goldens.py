@@ -8,6 +8,7 @@ tolerance, so its result is computed once here and a sample is stored:
   python tests/golden/make_goldens.py cfg3                whole config 3 (128x128x64, S16, P3, 19 groups), closure 1
   python tests/golden/make_goldens.py cfg4 --source 0     config 4 (256x256x128, S8, P3, 47 groups), one of its 8 sources
   python tests/golden/make_goldens.py cfg4 --source 3     (source 0 is axis-aligned, source 3 sits at 135 degrees)
+  python tests/golden/make_goldens.py cfg4 --source 0 --closure 0   (pure diamond difference, reported beside the gate)
 
 Stored per (config, source) in tests/golden/<name>.npz, everything straight from oracle.solve (BASELINE.json configs[3],
 [4]; readings R8-R10 of DESIGN.md: the sweep counts K[g] are replayed on the GPU):
@@ -39,8 +40,8 @@ STRIDE = {3: 1021, 4: 4099}          # primes: the sample walks through every x,
 N_SMALL, N_LARGE = 2048, 256
 
 
-def golden_name(cfg, source):
-    return "cfg%d_src%d_closure1.npz" % (cfg, source)
+def golden_name(cfg, source, closure=1):
+    return "cfg%d_src%d_closure%d.npz" % (cfg, source, closure)
 
 
 def main():
@@ -48,6 +49,8 @@ def main():
     ap.add_argument("config", choices=["cfg3", "cfg4"])
     ap.add_argument("--source", type=int, default=0)
     ap.add_argument("--threads", type=int, default=0)
+    ap.add_argument("--closure", type=int, default=1, help="1 = diamond difference + set-to-zero fix-up (reading R2, the gate of "
+                    "configs 2-4); 0 = pure diamond difference (PAPER.md:287), stored beside it as a finding")
     args = ap.parse_args()
     cfg = int(args.config[3])
     wl = make_config(cfg)
@@ -61,8 +64,8 @@ def main():
     def progress(p, g, k, delta):
         print("  group %2d  sweeps %2d  delta %.3e  [%.0f s]" % (g, k, delta, time.time() - t0), flush=True)
 
-    print("%s source %d: oracle.solve, closure 1, tol %g, %d threads" % (wl.name, args.source, wl.tol, threads), flush=True)
-    res = oracle.solve(wl, closure=1, threads=threads, progress=progress,
+    print("%s source %d: oracle.solve, closure %d, tol %g, %d threads" % (wl.name, args.source, args.closure, wl.tol, threads), flush=True)
+    res = oracle.solve(wl, closure=args.closure, threads=threads, progress=progress,
                        store_dtype=np.float32 if cfg == 4 else np.float64)
     phi, phi_u = res["phi"][0], res["phi_u"][0]               # [G][nm][cells], [G][cells]
     G = wl.G
@@ -87,7 +90,7 @@ def main():
         small_idx.append(lo); small_phi.append(p0[lo]); large_idx.append(hi); large_phi.append(p0[hi])
     out.update(small_idx=np.stack(small_idx).astype(np.int32), small_phi0=np.stack(small_phi).astype(np.float32),
                large_idx=np.stack(large_idx).astype(np.int32), large_phi0=np.stack(large_phi).astype(np.float32))
-    path = os.path.join(HERE, golden_name(cfg, args.source))
+    path = os.path.join(HERE, golden_name(cfg, args.source, args.closure))
     np.savez_compressed(path, **out)
     print("wrote %s (%.1f KB) after %.0f s; sweeps per group %s" % (path, os.path.getsize(path) / 1024.0, time.time() - t0,
                                                                     out["iters"].tolist()), flush=True)

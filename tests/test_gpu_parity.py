@@ -47,11 +47,12 @@ def test_schedule_bit_exact(pkg, orc, wl_fn, brick):
     p.close()
 
 
-@pytest.mark.parametrize("brick", [(16, 8, 4), (8, 4, 8), (4, 3, 5), (12, 32, 1), (4, 1, 1)])
+@pytest.mark.parametrize("brick", [(16, 8, 4), (20, 8, 4), (8, 4, 8), (4, 3, 5), (12, 32, 1), (12, 1, 32), (4, 1, 1), (64, 8, 4)])
 def test_device_wavefront_planes_bit_exact(pkg, orc, brick):
     """Level 2 on the device: the step at which the sweep kernel itself updates each cell of a brick
     equals the cell's sub-sweep index of Eq. (8) in the oracle's schedule, for all 8 octants, and every
-    plane holds exactly P(S) cells (Eq. 9)."""
+    plane holds exactly P(S) cells (Eq. 9).  The same launch bounds-checks every shared-memory address of the
+    wavefront loop (idle lanes load from their running addresses): the call fails if one leaves the CTA's allocation."""
     p = pkg.problem_from_workload(make_config(0))
     bx, by, bz = brick
     for octant in range(8):
