@@ -12,6 +12,8 @@
 #include <string>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>
+
 #include "device_common.cuh"
 #include "host_tables.h"
 #include "kernels.cuh"
@@ -120,6 +122,14 @@ struct doctors_problem {
 };
 
 namespace {
+
+// NVTX range around a phase of doctors_solve (host side; shows up in nsys / ncu timelines, costs nothing without a tool)
+struct NvtxRange {
+    explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+    NvtxRange(const NvtxRange&) = delete;
+    NvtxRange& operator=(const NvtxRange&) = delete;
+};
 
 int fail(doctors_problem* p, int code, const char* fmt, ...)
 {
@@ -1064,6 +1074,7 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         }
     }
 
+    NvtxRange nvtx_solve("doctors_solve");
     CK(cudaEventRecord(ev_total0, st));
     for (int ch = 0; ch < P.nchunks; ++ch) {
         const int prob0 = ch * P.chunk;
@@ -1073,6 +1084,8 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         float* phi_u_c = at<float>(p, P.o_phiu) + (size_t)src0 * G * cp;
 
         // a1: uncollided flux of the chunk's sources
+        {
+        NvtxRange nvtx_ray("a1 raytrace");
         CK(cudaEventRecord(ev_a, st));
         k_raytrace<<<dim3(unsigned((P.cells_p + kRayThreads - 1) / kRayThreads), nsrc_c), kRayThreads, 0, st>>>(
             md, at<uint8_t>(p, P.o_matd), at<float>(p, P.o_rhod), at<SourceDev>(p, P.o_srcs), src0,
@@ -1082,9 +1095,11 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
         CK(cudaEventRecord(ev_b, st));
         CK(cudaEventSynchronize(ev_b));
         { float ms = 0; cudaEventElapsedTime(&ms, ev_a, ev_b); ms_ray += ms; }
+        }
 
         int prev_group_iters = 0;                                 // sweeps the previous group of this chunk needed
         for (int g = 0; g < G; ++g) {
+            NvtxRange nvtx_group("group: a2 fixed source + a6 source iteration (a3-a5 sweeps)");
             k_group_begin<<<1, 256, 0, st>>>(at<ProbState>(p, P.o_state), at<Control>(p, P.o_ctl), at<int>(p, P.o_fixediters),
                                               prob0, nq, P.chunk, G, g, at<double>(p, P.o_bal));
             k_sigt<<<cblocks, 256, 0, st>>>(md, at<uint8_t>(p, P.o_mat), at<float>(p, P.o_rho), at<double>(p, P.o_sigt_hat), G, g, at<double>(p, P.o_sigt));

@@ -180,3 +180,36 @@ def test_total_balance_with_first_collision_source(orc):
     absorbed = ((sig_t - sig_s0) * phi0).sum() * V
     leak = res["balance"][0, 0, 2]
     assert abs(first - absorbed - leak) < 1e-8 * first
+
+
+@pytest.mark.parametrize("pos", [(0.9, -0.55, 0.4), (-9.3, 2.1, -1.7)])
+def test_four_material_mesh_against_fine_sampling_source_inside_and_outside(orc, pos):
+    """The oracle's voxel traversal and the library's ray-trace kernel are the same textbook algorithm (parametric
+    stepping), so GPU-vs-oracle parity cannot catch an error both share.  This pin is structurally different: the areal
+    density per material along source -> cell centre by a dumb midpoint rule (200000 samples, voxel looked up by floor),
+    on the ragged four-material mesh of the GPU tests, pitch different per axis, with the source inside the mesh (no clipping,
+    t0 = 0) and outside it (clipped entry through a face)."""
+    from tests.parity_util import tiny_p3_case
+    wl = tiny_p3_case()
+    src = SourceSpec(kind=1, pos=pos, spectrum=np.full(wl.G, 1.0 / wl.G))
+    _, areal = orc.raytrace(wl, src, want_areal=True)
+    rho = wl.density.astype(float).reshape(-1)
+    mat = wl.material.reshape(-1)
+    d = np.array([wl.dx, wl.dy, wl.dz]); n = np.array([wl.nx, wl.ny, wl.nz])
+    lo = -0.5 * n * d
+    rng = np.random.default_rng(5)
+    ns = 200000
+    t = (np.arange(ns) + 0.5) / ns
+    for c in rng.integers(0, wl.cells, 30):
+        ijk = np.array([c % wl.nx, (c // wl.nx) % wl.ny, c // (wl.nx * wl.ny)])
+        rc = lo + (ijk + 0.5) * d
+        seg = rc - np.array(pos)
+        R = np.linalg.norm(seg)
+        p = np.array(pos)[None, :] + t[:, None] * seg[None, :]
+        idx = np.floor((p - lo) / d).astype(int)
+        ok = ((idx >= 0) & (idx < n)).all(1)
+        cc = idx[ok, 0] + wl.nx * (idx[ok, 1] + wl.ny * idx[ok, 2])
+        for m in range(wl.n_materials):
+            a = (rho[cc] * (mat[cc] == m)).sum() * R / ns
+            assert abs(a - areal[m, c]) < 3e-4 * max(1.0, areal[:, c].sum()) + 2e-5, (c, m, a, areal[m, c])
+        assert areal[:, c].sum() > 0
