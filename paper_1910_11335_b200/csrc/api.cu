@@ -1137,8 +1137,8 @@ extern "C" int doctors_solve(doctors_problem* p, const doctors_solve_opts* opts_
                     batch = std::min(limit - k, k == 0 ? (prev_group_iters > 1 ? prev_group_iters - 1 : std::min(o.check_window, 6)) : 1);
                 for (int b = 0; b < batch; ++b, ++k) {
 #define LAUNCH_UPDATE(NMv)                                                                                          \
-    k_update<NMv><<<dim3(cblocks, nq), 256, 0, st>>>(md, at<uint8_t>(p, P.o_mat), at<float>(p, P.o_rho), at<float>(p, P.o_sigs), \
-        L, G, g, G, k == 0 ? 1 : 0, at<float>(p, P.o_fixed), at<float>(p, P.o_phiall), at<float>(p, P.o_Q),          \
+    k_update<NMv><<<dim3((cblocks + 3) / 4, nq), 256, 0, st>>>(md, at<uint8_t>(p, P.o_mat), at<float>(p, P.o_rho), at<float>(p, P.o_sigs), \
+        p->n_mat_xs, L, G, g, G, k == 0 ? 1 : 0, at<float>(p, P.o_fixed), at<float>(p, P.o_phiall), at<float>(p, P.o_Q),          \
         at<float>(p, P.o_phi0old), at<ProbState>(p, P.o_state), at<Control>(p, P.o_ctl), at<double>(p, P.o_leak))
                     switch (NM) { case 1: LAUNCH_UPDATE(1); break; case 4: LAUNCH_UPDATE(4); break; case 9: LAUNCH_UPDATE(9); break; default: LAUNCH_UPDATE(16); }
 #undef LAUNCH_UPDATE

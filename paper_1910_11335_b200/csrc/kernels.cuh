@@ -199,7 +199,8 @@ k_fixed_source(MeshDev m, const uint8_t* __restrict__ mat, const float* __restri
     }
     // downscatter from the finished groups g' < g
     const float* pa = phi_all + (size_t)p * G * NM * m.cells_p + cp;
-    for (int gp = 0; gp < g; ++gp) {
+#pragma unroll 2
+    for (int gp = 0; gp < g; ++gp) {                   // 2 x NM independent loads in flight per thread (streaming, HBM-bound)
         float sl[4];
 #pragma unroll
         for (int l = 0; l < 4; ++l) sl[l] = l <= L ? dens * ss[l * ng + gp] : 0.0f;
@@ -219,37 +220,48 @@ k_fixed_source(MeshDev m, const uint8_t* __restrict__ mat, const float* __restri
 template <int NM>
 __global__ void __launch_bounds__(256)
 k_update(MeshDev m, const uint8_t* __restrict__ mat, const float* __restrict__ rho,
-         const float* __restrict__ sig_s, int L, int G, int g, int Gs /*group slots in phi*/, int first,
+         const float* __restrict__ sig_s, int n_mat, int L, int G, int g, int Gs /*group slots in phi*/, int first,
          const float* __restrict__ fixed, float* __restrict__ phi /*[prob][Gs][NM][cells_p] at group g*/,
          float* __restrict__ Q, float* __restrict__ phi0_old, const ProbState* __restrict__ st,
          Control* ctl, double* leak)
 {
+    // four consecutive cells per thread: 16-byte loads and stores on every plane (cells_p is a multiple of 4: BX is)
+    __shared__ float s_self[kMaxMaterials * 4];        // s_l[mat][g -> g]
     const int p = blockIdx.y;
     if (blockIdx.x == 0 && threadIdx.x < 10) {
         if (p == 0) ctl->counters[threadIdx.x] = 0u;
         if (threadIdx.x == 0 && !st[p].done) leak[p] = 0.0;
     }
     if (st[p].done) return;
-    long long cp = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (cp >= m.cells_p) return;
-    float* ph = phi + ((size_t)p * Gs + g) * NM * m.cells_p + cp;
-    float* q = Q + (size_t)p * NM * m.cells_p + cp;
-    const float* fx = fixed + (size_t)p * NM * m.cells_p + cp;
-    const float dens = rho[cp];                                   // padding cells: density 0, fixed 0 -> Q = 0
-    const int mt = mat[cp];
-    float sl[4];
-#pragma unroll
-    for (int l = 0; l < 4; ++l) sl[l] = l <= L ? dens * sig_s[(((size_t)mt * (L + 1) + l) * G + g) * G + g] : 0.0f;
-    float p0 = 0.0f;
+    for (int t = threadIdx.x; t < n_mat * 4; t += blockDim.x) {
+        const int mt = t >> 2, l = t & 3;
+        s_self[t] = l <= L ? sig_s[(((size_t)mt * (L + 1) + l) * G + g) * G + g] : 0.0f;
+    }
+    __syncthreads();
+    const long long c4 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * 4;
+    if (c4 >= m.cells_p) return;
+    float* ph = phi + ((size_t)p * Gs + g) * NM * m.cells_p + c4;
+    float* q = Q + (size_t)p * NM * m.cells_p + c4;
+    const float* fx = fixed + (size_t)p * NM * m.cells_p + c4;
+    const float4 dens = *reinterpret_cast<const float4*>(rho + c4);          // padding cells: density 0, fixed 0 -> Q = 0
+    const uchar4 mt = *reinterpret_cast<const uchar4*>(mat + c4);
+    float4 p0 = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
 #pragma unroll
     for (int lm = 0; lm < NM; ++lm) {
-        float f = fx[(size_t)lm * m.cells_p];
-        float v = first ? 0.0f : ph[(size_t)lm * m.cells_p];
+        const int l = l_of_lm(lm);
+        const float4 f = *reinterpret_cast<const float4*>(fx + (size_t)lm * m.cells_p);
+        float4 v = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        if (!first) v = *reinterpret_cast<const float4*>(ph + (size_t)lm * m.cells_p);
         if (lm == 0) p0 = v;
-        q[(size_t)lm * m.cells_p] = fmaf(sl[l_of_lm(lm)], v, f);
-        ph[(size_t)lm * m.cells_p] = 0.0f;
+        float4 o;
+        o.x = fmaf(dens.x * s_self[mt.x * 4 + l], v.x, f.x);
+        o.y = fmaf(dens.y * s_self[mt.y * 4 + l], v.y, f.y);
+        o.z = fmaf(dens.z * s_self[mt.z * 4 + l], v.z, f.z);
+        o.w = fmaf(dens.w * s_self[mt.w * 4 + l], v.w, f.w);
+        *reinterpret_cast<float4*>(q + (size_t)lm * m.cells_p) = o;
+        *reinterpret_cast<float4*>(ph + (size_t)lm * m.cells_p) = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
     }
-    phi0_old[(size_t)p * m.cells_p + cp] = p0;
+    *reinterpret_cast<float4*>(phi0_old + (size_t)p * m.cells_p + c4) = p0;
 }
 
 // a6  End of iteration k: delta_k = max|phi_00^k - phi_00^(k-1)| / max|phi_00^k| per problem (reading R8);
