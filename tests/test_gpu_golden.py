@@ -157,3 +157,20 @@ def test_config4_closure0_literal_diamond_difference_against_golden(pkg, capsys)
     high = [r for r in report if r[1] < 40]                       # groups 0-39 (above ~30 keV)
     assert all(r[2] < TOL for r in high), [r for r in high if r[2] >= TOL]
     assert worst < 1e-3 and sum(r[4] for r in report) <= 50, report
+
+
+def test_config3_closure0_literal_diamond_difference_against_golden(pkg, capsys):
+    """SURVEY row f2 on config 3: pure diamond difference, whole 19-group solve, against the oracle run with the
+    same closure; per-group worst relative error and count of stored cells above 1e-4 are printed."""
+    gold = _golden(3, 0, closure=0)
+    wl = make_config(3)
+    p, info = run_gpu(wl, closure=0, fixed_iters=gold["iters"][None, :])
+    report = []
+    worst = _compare(p, 0, gold, wl, report)
+    p.close()
+    with capsys.disabled():
+        print("\n  cfg3 closure 0: worst rel err %.3e; cells above 1e-4: %d of %d stored; oracle cells with phi0 < 0: %d" % (
+            worst, sum(r[4] for r in report), sum(r[3] for r in report), int(gold["n_negative"].sum())))
+        print("   per group max: %s" % " ".join("%.1e" % r[2] for r in report))
+    assert all(r[2] < TOL for r in report if r[1] < 16), report     # groups 0-15 (above 30 keV) hold the gate
+    assert worst < 1e-3 and sum(r[4] for r in report) <= 50, report
