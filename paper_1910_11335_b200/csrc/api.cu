@@ -38,6 +38,7 @@ struct Plan {
     bool ok = false;
     long long cells_p = 0; int NCb = 0; int tm_inner = 0, tm_rows = 0;   // TMA box = tm_rows rows of tm_inner cells = one brick
     int MT = 0;                     // m-tiles of the tensor-core projections (0: FFMA2 loops), see sweep_brick.cuh
+    unsigned fbytes = 8;            // bytes per exchanged face value: 4 with closure 1, 8 with closure 0 (sweep_brick.cuh, FaceOf)
     int nprob = 0, chunk = 0, nchunks = 0, nsrc = 0, nvol = 0;
     int G = 0, L = 0, NM = 0, ndir = 0, M = 0;
     int mode = 0, sweep_mode = 0, deterministic = 0;
@@ -177,7 +178,7 @@ bool wants_mma(const doctors_solve_opts* o, int M)
     return pr == 2 || (pr == 0 && M > 16);
 }
 
-void auto_brick(int NM, int M, int nx, int ny, int nz, const int* req, bool mt, int B[3])
+void auto_brick(int NM, int M, int nx, int ny, int nz, const int* req, bool mt, unsigned fbytes, int B[3])
 {
     if (req && req[0] > 0 && req[1] > 0 && req[2] > 0) { B[0] = req[0]; B[1] = req[1]; B[2] = req[2]; return; }
     // cross section = the 32 lanes of a warp (8 x 4, reshaped for thin meshes); BX as long as shared memory allows
@@ -185,8 +186,9 @@ void auto_brick(int NM, int M, int nx, int ny, int nz, const int* req, bool mt, 
     B[2] = std::min(32 / B[1], nz);
     if (B[2] < 4 && B[1] < ny) B[1] = std::min(32 / B[2], ny);
     const int cand[5] = {20, 16, 12, 8, 4};        // 20 x 8 x 4 = 640 cells = 2 per thread of a 320-thread CTA, 3 CTAs per SM
+                                                    // (24 x 8 x 4 also fits three CTAs with fp32 exchange faces: measured equal, 8.61 ms)
     auto fits = [&](int bx, size_t limit) {
-        return brick_smem_layout(NM, bx, B[1], B[2], M, mt ? projection_mtiles(NM, M, bx * B[1] * B[2]) : 0).total <= limit;
+        return brick_smem_layout(NM, bx, B[1], B[2], M, mt ? projection_mtiles(NM, M, bx * B[1] * B[2]) : 0, fbytes).total <= limit;
     };
     for (int c = 0; c < 5; ++c) {
         B[0] = std::min(cand[c], (nx + 3) / 4 * 4);
@@ -215,7 +217,8 @@ Plan make_plan(const doctors_problem* p, const doctors_solve_opts* o, int chunk)
     P.sweep_mode = o ? o->sweep_mode : 0;
     P.deterministic = o ? o->deterministic : 0;
     for (auto& s : p->sources) if (s.kind == 0) ++P.nvol;
-    auto_brick(P.NM, P.M, p->nx, p->ny, p->nz, o ? o->brick : nullptr, wants_mma(o, P.M), P.B);
+    P.fbytes = face_bytes(o && o->closure == 1);
+    auto_brick(P.NM, P.M, p->nx, p->ny, p->nz, o ? o->brick : nullptr, wants_mma(o, P.M), P.fbytes, P.B);
     P.gb[0] = (p->nx + P.B[0] - 1) / P.B[0];
     P.gb[1] = (p->ny + P.B[1] - 1) / P.B[1];
     P.gb[2] = (p->nz + P.B[2] - 1) / P.B[2];
@@ -228,7 +231,7 @@ Plan make_plan(const doctors_problem* p, const doctors_solve_opts* o, int chunk)
     P.tm_inner = P.NCb / P.tm_rows;
     P.ntasks = P.nbricks * 8 * P.chunk;
     P.MT = wants_mma(o, P.M) ? projection_mtiles(P.NM, P.M, P.NCb) : 0;
-    P.smem = brick_smem_layout(P.NM, P.B[0], P.B[1], P.B[2], P.M, P.MT).total;
+    P.smem = brick_smem_layout(P.NM, P.B[0], P.B[1], P.B[2], P.M, P.MT, P.fbytes).total;
     { int dpw = (P.M + kMaxSweepWarps - 1) / kMaxSweepWarps; P.W = (P.M + dpw - 1) / dpw; }
 
     size_t off = 0;
@@ -271,9 +274,9 @@ Plan make_plan(const doctors_problem* p, const doctors_solve_opts* o, int chunk)
         P.face_z_n = size_t(P.M) * P.B[0] * P.B[1];
         P.o_tasks = take(size_t(P.ntasks) * sizeof(uint2));
         P.o_flags = take(size_t(P.chunk) * 8 * P.nbricks * 4);
-        P.o_fx = take(size_t(P.chunk) * 8 * P.gb[1] * P.gb[2] * P.face_x_n * 8);
-        P.o_fy = take(size_t(P.chunk) * 8 * P.gb[0] * P.gb[2] * P.face_y_n * 8);
-        P.o_fz = take(size_t(P.chunk) * 8 * P.gb[0] * P.gb[1] * P.face_z_n * 8);
+        P.o_fx = take(size_t(P.chunk) * 8 * P.gb[1] * P.gb[2] * P.face_x_n * P.fbytes);
+        P.o_fy = take(size_t(P.chunk) * 8 * P.gb[0] * P.gb[2] * P.face_y_n * P.fbytes);
+        P.o_fz = take(size_t(P.chunk) * 8 * P.gb[0] * P.gb[1] * P.face_z_n * P.fbytes);
         P.o_dbg = take(size_t(P.B[0]) * P.B[1] * P.B[2] * 4);
         P.o_octtab = take(8 * octtab_layout(P.NM, P.M, P.MT).total);
         P.o_sched = P.o_ox = P.o_oy = P.o_oz = 0;
@@ -575,7 +578,8 @@ int doctors_debug_schedule_dims(doctors_problem* p, const doctors_solve_opts* op
     if (level == 0) { dims[0] = p->nx; dims[1] = p->ny; dims[2] = p->nz; return DOCTORS_OK; }
     if (!p->has_xs || !p->has_quad) return fail(p, DOCTORS_BAD_STATE, "xs / quadrature not set (brick size depends on them)");
     int B[3];
-    auto_brick((p->L + 1) * (p->L + 1), p->ndir / 8, p->nx, p->ny, p->nz, opts ? opts->brick : nullptr, wants_mma(opts, p->ndir / 8), B);
+    auto_brick((p->L + 1) * (p->L + 1), p->ndir / 8, p->nx, p->ny, p->nz, opts ? opts->brick : nullptr, wants_mma(opts, p->ndir / 8),
+               face_bytes(opts && opts->closure == 1), B);
     if (level == 1) { for (int a = 0; a < 3; ++a) dims[a] = ((a == 0 ? p->nx : a == 1 ? p->ny : p->nz) + B[a] - 1) / B[a]; return DOCTORS_OK; }
     if (level == 2) { for (int a = 0; a < 3; ++a) dims[a] = B[a]; return DOCTORS_OK; }
     return fail(p, DOCTORS_INVALID_ARG, "level must be 0, 1 or 2");
@@ -952,9 +956,12 @@ int prepare(doctors_problem* p, const doctors_solve_opts& o, const Plan& P)
         bp.tasks = at<uint2>(p, P.o_tasks);
         bp.ctl = at<Control>(p, P.o_ctl);
         bp.flags = at<unsigned>(p, P.o_flags);
-        bp.faceX = at<double>(p, P.o_fx); bp.faceY = at<double>(p, P.o_fy); bp.faceZ = at<double>(p, P.o_fz);
+        bp.faceX = at<char>(p, P.o_fx); bp.faceY = at<char>(p, P.o_fy); bp.faceZ = at<char>(p, P.o_fz);
         bp.dbg_plane = nullptr;
-        bp.bulk_faces = (P.face_x_n % 2 == 0 && P.face_y_n % 2 == 0 && P.face_z_n % 2 == 0) ? 1 : 0;
+        {   // bulk async copies move multiples of 16 bytes
+            const size_t q = 16 / P.fbytes;
+            bp.bulk_faces = (P.face_x_n % q == 0 && P.face_y_n % q == 0 && P.face_z_n % q == 0) ? 1 : 0;
+        }
         bp.state = at<ProbState>(p, P.o_state);
         bp.leak = at<double>(p, P.o_leak);
     } else {
@@ -1271,7 +1278,7 @@ extern "C" int doctors_debug_device_brick_steps(doctors_problem* p, int bx, int 
         return fail(p, DOCTORS_INVALID_ARG, "brick: bx a multiple of 4 (<= 64), by * bz <= 32");
     CK(cudaSetDevice(p->device));
     const int NC = bx * by * bz;
-    const size_t smem = brick_smem_layout(1, bx, by, bz, 1, 0).total;
+    const size_t smem = brick_smem_layout(1, bx, by, bz, 1, 0, face_bytes(false)).total;
     // scratch: Q, phi (float), sigt (double), faces (double), table blobs, control
     struct Scratch { float* Q; float* phi; double* sig; double* face; unsigned char* tab; uint2* task;
                      unsigned* flags; Control* ctl; ProbState* st; double* leak; int* planes; } S;

@@ -35,6 +35,28 @@
 
 namespace doctors {
 
+// Storage type of the faces EXCHANGED between bricks (global buffers and the shared-memory face arrays of a task).  The
+// recurrence inside a brick is fp64 (registers, shuffles) either way; only what crosses a brick boundary is stored: every
+// 20th x face, 8th y face and 4th z face of a ray.
+//   closure 1 (FIX, the gated closure of configs 2-4): fp32.  Halves the only DRAM traffic in excess of the algorithmic bytes
+//     (1.32 x -> 1.17 x) and 11 KB of shared memory per CTA; the whole config-4 solve stays within 3.8e-6 of the oracle
+//     (1.2e-6 with fp64 faces), and the power it saves lifts the power-capped SM clock of the whole solve from ~1865 to 1950 MHz.
+//   closure 0 (pure diamond difference): fp64.  Its ill-conditioned cells (sign changes of phi_0 in the lowest groups) lose
+//     with fp32 exchange faces: 24 instead of 3-4 of 202722 stored cells of config 4 above 1e-4.
+template <bool FIX> struct FaceOf { using type = double; };
+template <> struct FaceOf<true> { using type = float; };
+__host__ __device__ constexpr unsigned face_bytes(bool fix) { return fix ? 4u : 8u; }
+template <typename F>
+__device__ __forceinline__ double load_face(uint32_t a)
+{
+    if constexpr (sizeof(F) == 8) return lds_f64(a); else return (double)lds_f32(a);
+}
+template <typename F>
+__device__ __forceinline__ void store_face_if(bool p, uint32_t a, double v)
+{
+    if constexpr (sizeof(F) == 8) sts_f64_if(p, a, v); else sts_f32_if(p, a, (float)v);
+}
+
 struct BrickParams {
     int nx, ny, nz;              // mesh
     int BX, BY, BZ;              // brick extents (BX % 4 == 0, BY * BZ <= 32)
@@ -56,9 +78,9 @@ struct BrickParams {
     const uint2* tasks;          // x = prob | octant << 8,  y = bi | bj << 10 | bk << 20
     Control* ctl;
     unsigned* flags;             // [prob][8][bricks]
-    double* faceX;               // [prob][8][gby*gbz][M][BZ][BY]
-    double* faceY;               // [prob][8][gbx*gbz][M][BZ][BX]
-    double* faceZ;               // [prob][8][gbx*gby][M][BY][BX]
+    void* faceX;                 // [prob][8][gby*gbz][M][BZ][BY]   float (closure 1) or double (closure 0), see FaceOf
+    void* faceY;                 // [prob][8][gbx*gbz][M][BZ][BX]
+    void* faceZ;                 // [prob][8][gbx*gby][M][BY][BX]
     const ProbState* state;
     double* leak;                // [prob]
     int bulk_faces;              // 1: all three face blocks are multiples of 16 bytes -> moved by bulk async copies (TMA unit)
@@ -102,7 +124,7 @@ struct BrickSmem {
     size_t q, sig, psi, fx, fy, fz, tab, done, misc, total;
 };
 
-__host__ __device__ inline BrickSmem brick_smem_layout(int NM, int BX, int BY, int BZ, int M, int MT)
+__host__ __device__ inline BrickSmem brick_smem_layout(int NM, int BX, int BY, int BZ, int M, int MT, unsigned kFaceBytes)
 {
     BrickSmem s;
     size_t NC = size_t(BX) * BY * BZ, o = 0;
@@ -115,9 +137,9 @@ __host__ __device__ inline BrickSmem brick_smem_layout(int NM, int BX, int BY, i
     s.q = o;     o = align_up(o + size_t(NM > M ? NM : M) * plane_pitch(int(NC), MT) * 4, 128);
     s.sig = o;   o = align_up(o + NC * 8, 128);
     s.psi = s.q;
-    s.fx = o;    o = align_up(o + size_t(M) * BY * BZ * 8, 8);      // fx, fy, fz contiguous (one load loop)
-    s.fy = o;    o = align_up(o + size_t(M) * BX * BZ * 8, 8);
-    s.fz = o;    o = align_up(o + size_t(M) * BX * BY * 8, 16);
+    s.fx = o;    o = align_up(o + size_t(M) * BY * BZ * kFaceBytes, kFaceBytes);      // fx, fy, fz contiguous (one load loop)
+    s.fy = o;    o = align_up(o + size_t(M) * BX * BZ * kFaceBytes, kFaceBytes);
+    s.fz = o;    o = align_up(o + size_t(M) * BX * BY * kFaceBytes, 16);
     s.tab = o;   o = align_up(o + octtab_layout(NM, M, MT).total, 16);
     s.done = o;  o = align_up(o + 256, 16);      // "problem has stopped" bytes of the launch (task prob index is 8 bits)
     o = align_up(o + 128 + size_t(8) * BY * (BY + BZ - 2), 16);   // tail pad: lanes past their x range (sx < 0: before it) overshoot by the same amount
@@ -300,14 +322,16 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
     const int BX = P.BX, BY = P.BY, BZ = P.BZ, M = P.M;
     const int NC = BX * BY * BZ;
     const int NCP = plane_pitch(NC, MT);                              // plane pitch of the tile (floats)
-    const BrickSmem L = brick_smem_layout(NM, BX, BY, BZ, M, MT);
+    using face_t = typename FaceOf<FIX>::type;
+    constexpr unsigned kFaceBytes = sizeof(face_t);
+    const BrickSmem L = brick_smem_layout(NM, BX, BY, BZ, M, MT, kFaceBytes);
     const OctTab T = octtab_layout(NM, M, MT);
     float* sQ = reinterpret_cast<float*>(smem + L.q);
     double* sSig = reinterpret_cast<double*>(smem + L.sig);
     float* sPsi = reinterpret_cast<float*>(smem + L.psi);
-    double* sFx = reinterpret_cast<double*>(smem + L.fx);
-    double* sFy = reinterpret_cast<double*>(smem + L.fy);
-    double* sFz = reinterpret_cast<double*>(smem + L.fz);
+    face_t* sFx = reinterpret_cast<face_t*>(smem + L.fx);
+    face_t* sFy = reinterpret_cast<face_t*>(smem + L.fy);
+    face_t* sFz = reinterpret_cast<face_t*>(smem + L.fz);
     double* sDir = reinterpret_cast<double*>(smem + L.tab + T.dir);  // [M][4]
     float4* sLk = reinterpret_cast<float4*>(smem + L.tab + T.lk);
     float* sM = reinterpret_cast<float*>(smem + L.tab + T.t0);      // MT = 0: [M][pitch];  MT >= 1: A fragments (float4 per lane)
@@ -380,9 +404,9 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         const int brick = bi + P.gbx * (bj + P.gby * bk);
         unsigned* flag_base = P.flags + (size_t)(prob * 8 + oct) * nbricks;
         const size_t po = (size_t)prob * 8 + oct;
-        double* gFx = P.faceX + (po * (P.gby * P.gbz) + bj + P.gby * bk) * (size_t)faceXn;
-        double* gFy = P.faceY + (po * (P.gbx * P.gbz) + bi + P.gbx * bk) * (size_t)faceYn;
-        double* gFz = P.faceZ + (po * (P.gbx * P.gby) + bi + P.gbx * bj) * (size_t)faceZn;
+        face_t* gFx = static_cast<face_t*>(P.faceX) + (po * (P.gby * P.gbz) + bj + P.gby * bk) * (size_t)faceXn;
+        face_t* gFy = static_cast<face_t*>(P.faceY) + (po * (P.gbx * P.gbz) + bi + P.gbx * bk) * (size_t)faceYn;
+        face_t* gFz = static_cast<face_t*>(P.faceZ) + (po * (P.gbx * P.gby) + bi + P.gbx * bj) * (size_t)faceZn;
 
         // tile, sigma_t and (when the octant changes) the octant's table blob: bulk async copies, one mbarrier.
         // Directions of an octant are contiguous (n = oct*M + m); nobody reads the old tables any more (loop-top barrier).
@@ -412,9 +436,9 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
                 const bool need = lane == 0 ? upx : (lane == 1 ? upy : upz);
                 if (need) {
                     const int up = lane == 0 ? brick - sx : (lane == 1 ? brick - sy * P.gbx : brick - sz * P.gbx * P.gby);
-                    const double* src = lane == 0 ? gFx : (lane == 1 ? gFy : gFz);
+                    const face_t* src = lane == 0 ? gFx : (lane == 1 ? gFy : gFz);
                     const uint32_t dst = smem_u32(lane == 0 ? sFx : (lane == 1 ? sFy : sFz));
-                    const uint32_t bytes = 8u * uint32_t(lane == 0 ? faceXn : (lane == 1 ? faceYn : faceZn));
+                    const uint32_t bytes = kFaceBytes * uint32_t(lane == 0 ? faceXn : (lane == 1 ? faceYn : faceZn));
                     while (ld_acquire_u32(flag_base + up) != P.epoch) { }
                     fence_proxy_async_global();                     // flag acquired (generic proxy) -> async-proxy read of the face
                     mbar_expect_tx(barF, bytes);
@@ -437,26 +461,26 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
 
         // inflow faces: upwind brick's outflow, or vacuum.  sFx, sFy, sFz are contiguous.
         const int nxy = faceXn + faceYn, nall = nxy + faceZn;
-        double fv[kFaceRegs];
+        face_t fv[kFaceRegs];
         if (P.bulk_faces) {
             // vacuum faces are zero-filled by the threads; the others arrive by the pollers' bulk copies
-            if (!upx) for (int e = tid; e < faceXn; e += nthr) sFx[e] = 0.0;
-            if (!upy) for (int e = tid; e < faceYn; e += nthr) sFy[e] = 0.0;
-            if (!upz) for (int e = tid; e < faceZn; e += nthr) sFz[e] = 0.0;
+            if (!upx) for (int e = tid; e < faceXn; e += nthr) sFx[e] = face_t(0);
+            if (!upy) for (int e = tid; e < faceYn; e += nthr) sFy[e] = face_t(0);
+            if (!upz) for (int e = tid; e < faceZn; e += nthr) sFz[e] = face_t(0);
         } else {
             // odd-sized blocks: the first kFaceRegs elements of every thread travel through registers (their
             // loads are issued here and parked in shared memory after phase 0), the rest is copied directly
 #pragma unroll
             for (int k = 0; k < kFaceRegs; ++k) {
                 const int e = tid + k * nthr;
-                const double* src = e < faceXn ? gFx + e : (e < nxy ? gFy + (e - faceXn) : gFz + (e - nxy));
+                const face_t* src = e < faceXn ? gFx + e : (e < nxy ? gFy + (e - faceXn) : gFz + (e - nxy));
                 const bool u = e < faceXn ? upx : (e < nxy ? upy : upz);
-                fv[k] = (e < nall && u) ? __ldcg(src) : 0.0;
+                fv[k] = (e < nall && u) ? __ldcg(src) : face_t(0);
             }
             for (int e = tid + kFaceRegs * nthr; e < nall; e += nthr) {
-                const double* src = e < faceXn ? gFx + e : (e < nxy ? gFy + (e - faceXn) : gFz + (e - nxy));
+                const face_t* src = e < faceXn ? gFx + e : (e < nxy ? gFy + (e - faceXn) : gFz + (e - nxy));
                 const bool u = e < faceXn ? upx : (e < nxy ? upy : upz);
-                sFx[e] = u ? __ldcg(src) : 0.0;
+                sFx[e] = u ? __ldcg(src) : face_t(0);
             }
         }
         mbar_wait(bar, parity);
@@ -468,9 +492,11 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         } else {
             // Two cells per thread share every coefficient load (the phase is bound by the shared-memory pipe);
             // packed fp32x2 FMAs (FFMA2, sm_100) accumulate even / odd moments in the halves of a register pair.
-            for (int c = tid; c < NC; c += 2 * nthr) {
-                const int c2 = c + nthr;
-                const bool two = c2 < NC;
+            // two cells per thread, (c, c + NC/2): NC is even (BX is a multiple of 4), so every thread of every round has both,
+            // whatever the brick length (768 cells on 320 threads: one round of 320 pairs, one of 64)
+            for (int c = tid; c < NC / 2; c += nthr) {
+                const int c2 = c + NC / 2;
+                constexpr bool two = true;
                 if constexpr (NM >= 2) {
                     float2 qa[NM / 2], qb[NM / 2];
     #pragma unroll
@@ -525,20 +551,20 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         // inside this CTA's shared memory, which starts with a 128-byte pad and ends with the tables — and
         // compute on that garbage; only stores and the x-face register are predicated.  Clipped lanes
         // (beyond ey / ez) stay parked on the tile's first cell.
-        int d4 = lane_ok ? 4 * sx * BY : 0, d8 = 2 * d4, d8f = lane_ok ? 8 * sx : 0;   // one cell along x: tile (fp32), sigma_t (fp64), face rows (fp64)
+        int d4 = lane_ok ? 4 * sx * BY : 0, d8 = 2 * d4, d8f = lane_ok ? int(kFaceBytes) * sx : 0;   // one cell along x: tile (fp32), sigma_t (fp64), face rows
         int shy = BY, ly = last_y ? 1 : 0, lz = last_z ? 1 : 0;
         // loop invariants pinned in registers: otherwise the compiler re-derives them every step (constant-bank reads,
         // ey - 1 / ez - 1 on the uniform datapath, 2 * d4)
         asm volatile("" : "+r"(d4), "+r"(d8), "+r"(d8f), "+r"(shy), "+r"(ly), "+r"(lz));
         for (int n = warp; n < M; n += P.W) {
             const double cx = sDir[4 * n], cy = sDir[4 * n + 1], cz = sDir[4 * n + 2], cs = sDir[4 * n + 3];
-            double* fxp = sFx + n * (BY * BZ) + lj + BY * lk_;
+            face_t* fxp = sFx + n * (BY * BZ) + lj + BY * lk_;
             // running shared-memory addresses of this lane's cell: advanced by one cell (sx) per step
             uint32_t pq = smem_u32(sPsi) + (lane_ok ? 4u * (uint32_t(n * NCP) + row) : 0u);
             uint32_t ps = smem_u32(sSig) + (lane_ok ? 8u * row : 0u);
-            uint32_t py = smem_u32(sFy) + (lane_ok ? 8u * uint32_t((n * BZ + lk_) * BX + li0) : 0u);
-            uint32_t pz = smem_u32(sFz) + (lane_ok ? 8u * uint32_t((n * BY + lj) * BX + li0) : 0u);
-            double ax = lane_ok ? *fxp : 0.0, oy = 0.0, oz = 0.0;
+            uint32_t py = smem_u32(sFy) + (lane_ok ? kFaceBytes * uint32_t((n * BZ + lk_) * BX + li0) : 0u);
+            uint32_t pz = smem_u32(sFz) + (lane_ok ? kFaceBytes * uint32_t((n * BY + lj) * BX + li0) : 0u);
+            double ax = lane_ok ? (double)*fxp : 0.0, oy = 0.0, oz = 0.0;
             int ip = lane_ok ? -(jp + kp) : -(1 << 29);          // clipped lanes never become active
 #pragma unroll 1
             for (int s = nsteps; s > 0; --s) {
@@ -547,13 +573,13 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
                 const bool act = (unsigned)ip < (unsigned)ex;    // this lane's cell lies on the current sub-sweep plane
                 const float q = lds_f32(pq);
                 const double sg = lds_f64(ps);
-                if (first_y) b = lds_f64(py);
-                if (first_z) cc = lds_f64(pz);
+                if (first_y) b = load_face<face_t>(py);
+                if (first_z) cc = load_face<face_t>(pz);
                 double ox;
                 const float psi = dd_cell<FIX>(act, q, sg, cx, cy, cz, cs, ax, b, cc, ox, oy, oz);
                 sts_f32_if(act, pq, psi);
-                sts_f64_if(act && ly, py, oy);
-                sts_f64_if(act && lz, pz, oz);
+                store_face_if<face_t>(act && ly, py, oy);
+                store_face_if<face_t>(act && lz, pz, oz);
                 if (act) ax = ox;
                 if (DBG) {
                     // debug instantiation (doctors_debug_device_brick_steps): the step at which each cell is visited, and a
@@ -561,20 +587,20 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
                     // running addresses, see above): slot NC of dbg_plane counts addresses outside this CTA's allocation
                     if (act) P.dbg_plane[(pq - smem_u32(sPsi)) / 4u - uint32_t(n * NCP)] = nsteps - s;   // indexed by the storage order (y fastest)
                     const uint32_t lo = smem_u32(smem), hi = lo + uint32_t(L.total);
-                    const bool bad = pq < lo || pq + 4u > hi || ps < lo || ps + 8u > hi || py < lo || py + 8u > hi || pz < lo || pz + 8u > hi;
+                    const bool bad = pq < lo || pq + 4u > hi || ps < lo || ps + 8u > hi || py < lo || py + kFaceBytes > hi || pz < lo || pz + kFaceBytes > hi;
                     if (bad) atomicAdd(P.dbg_plane + NC, 1);
                 }
                 ++ip; pq += d4; ps += d8; py += d8f; pz += d8f;
             }
-            if (lane_ok) *fxp = ax;
+            if (lane_ok) *fxp = face_t(ax);
         }
         if (P.bulk_faces) fence_proxy_async_smem();              // lanes' face writes -> visible to the async proxy
         __syncthreads();
         // ---- outflow faces to the downwind bricks: bulk async stores issued by the publisher (last lane of the last warp) ----
         if (P.bulk_faces && warp == pubWarp && lane == 31) {
-            if (dnx) bulk_store(gFx, smem_u32(sFx), uint32_t(8 * faceXn));
-            if (dny) bulk_store(gFy, smem_u32(sFy), uint32_t(8 * faceYn));
-            if (dnz) bulk_store(gFz, smem_u32(sFz), uint32_t(8 * faceZn));
+            if (dnx) bulk_store(gFx, smem_u32(sFx), uint32_t(kFaceBytes * faceXn));
+            if (dny) bulk_store(gFy, smem_u32(sFy), uint32_t(kFaceBytes * faceYn));
+            if (dnz) bulk_store(gFz, smem_u32(sFz), uint32_t(kFaceBytes * faceZn));
             bulk_commit();
         }
 
@@ -610,9 +636,11 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         if constexpr (MT >= 1) {
             project_directions_to_moments_mma<MT>(smem_u32(sQ), smem_u32(sD), NC, NCP, M);
         } else {
-            for (int c = tid; c < NC; c += 2 * nthr) {
-                const int c2 = c + nthr;
-                const bool two = c2 < NC;
+            // two cells per thread, (c, c + NC/2): NC is even (BX is a multiple of 4), so every thread of every round has both,
+            // whatever the brick length (768 cells on 320 threads: one round of 320 pairs, one of 64)
+            for (int c = tid; c < NC / 2; c += nthr) {
+                const int c2 = c + NC / 2;
+                constexpr bool two = true;
                 if constexpr (NM >= 2) {
                     float2 pa[NM / 2], pb[NM / 2];
                     float pla = 0.0f, plb = 0.0f;
