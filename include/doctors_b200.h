@@ -111,7 +111,9 @@ typedef struct {
     double tol;               /* stop when max|dphi_0| / max|phi_0| < tol (reading R8); <= 0 -> 1e-5 */
     int max_iters;            /* <= 0 -> 100 */
     const int* fixed_iters;   /* NULL, or [n_problems][G]: entry > 0 = exactly that many sweeps (R10) */
-    int closure;              /* 0 pure diamond difference; 1 + set-to-zero fix-up with rebalance (R2) */
+    int closure;              /* 0 pure diamond difference; 1 + set-to-zero fix-up with rebalance (R2).
+                               * The face recurrence is fp64 either way; faces that cross a brick boundary are stored as fp32 with
+                               * closure 1 and as fp64 with closure 0 */
     int deterministic;        /* 1: octants swept one after another, fixed summation order (bit-reproducible) */
     int source_chunk;         /* problems solved together (HBM capacity); 0 = all that fit the workspace */
     int sweep_mode;           /* 0 brick wavefront kernel (product path); 1 the paper's one-launch-per-sub-sweep scheme,

@@ -18,7 +18,7 @@
 // tensor-core projections, whose planes are padded, one 1-D bulk copy per moment plane instead —, 1-D bulk copies bring
 // sigma_t [brick] (fp64) and, when the CTA changes octant, the octant's table blob; phase 0 projects moments ->
 // directions (q_n, a5) for the whole brick; the wavefront phase applies the diamond-difference update (a4) in place
-// (q_n -> psi_n), its face recurrence in fp64; brick-to-brick faces go through global buffers (L2) guarded by
+// (q_n -> psi_n), its face recurrence in fp64; brick-to-brick faces (fp32 with closure 1, fp64 with closure 0: FaceOf) go through global buffers guarded by
 // release/acquire flags; phase 2 projects directions -> moments (Eq. 3) for the whole brick and one tensor reduce-add
 // (cp.reduce.async.bulk.tensor .add.f32) adds the tile into phi in L2 (so octants may touch a cell concurrently — the
 // paper's obstacle at PAPER.md:119).  The angular flux never leaves the SM.
