@@ -14,7 +14,7 @@ Stored per (config, source) in tests/golden/<name>.npz, everything straight from
 [4]; readings R8-R10 of DESIGN.md: the sweep counts K[g] are replayed on the GPU):
   iters [G], residual [G], balance [G][3], phi0_max [G], phi0_min [G], n_negative [G]
   stride_idx [S]                 cell indices i + nx (j + ny k) of a fixed stride sample (prime stride)
-  stride_phi [G][nm_s][S]        all moments (float32-rounded) of the collided flux there
+  stride_phi [G][nm_s][S]        all moments (float32-rounded) of the collided flux there (--lean: the scalar flux only)
   stride_phi_u [G][S]            uncollided flux there
   small_idx / small_phi0 [G][T]  the T smallest in-mask cells (phi0 > 1e-6 max phi0) of every group and their scalar flux:
                                  the relative error of an fp32 path peaks there
@@ -49,6 +49,8 @@ def main():
     ap.add_argument("config", choices=["cfg3", "cfg4"])
     ap.add_argument("--source", type=int, default=0)
     ap.add_argument("--threads", type=int, default=0)
+    ap.add_argument("--lean", action="store_true", help="store only the scalar flux on the stride sample (1.1 MB instead of 6.4 MB per "
+                    "config-4 source): used for the sources beyond 0, 3 and 5")
     ap.add_argument("--closure", type=int, default=1, help="1 = diamond difference + set-to-zero fix-up (reading R2, the gate of "
                     "configs 2-4); 0 = pure diamond difference (PAPER.md:287), stored beside it as a finding")
     args = ap.parse_args()
@@ -74,7 +76,7 @@ def main():
                phi0_max=np.array([phi[g, 0].max() for g in range(G)]), phi0_min=np.array([phi[g, 0].min() for g in range(G)]),
                n_negative=np.array([(phi[g, 0] < 0).sum() for g in range(G)], dtype=np.int64),
                stride_idx=sidx.astype(np.int32),
-               stride_phi=np.stack([phi[g][:, sidx] for g in range(G)]).astype(np.float32),
+               stride_phi=np.stack([phi[g][:1 if args.lean else None, sidx] for g in range(G)]).astype(np.float32),
                stride_phi_u=np.stack([phi_u[g][sidx] for g in range(G)]).astype(np.float32),
                mesh=np.array([wl.nx, wl.ny, wl.nz], dtype=np.int32), source=np.int32(args.source),
                seconds=np.array([res["seconds"][k] for k in ("raytrace", "fixed_source", "sweep")]),

@@ -101,7 +101,10 @@ def test_config4_full_solve_two_sources_against_golden(pkg, capsys):
     4.  Sources 0 (axis-aligned beam), 3 (135 degrees; both in the first chunk) and 5 (225 degrees, second chunk) replay the
     oracle's sweep counts through all 47 groups and are compared on every stored cell; the other five run the device-side
     convergence test in the same solve."""
-    golds = {s: _golden(4, s) for s in (0, 3, 5)}              # all required: tests/golden/make_goldens.py writes them
+    golds = {s: _golden(4, s) for s in (0, 3, 5)}              # required: tests/golden/make_goldens.py writes them
+    for s in range(8):                                         # the other sources where their (lean) golden is committed
+        if s not in golds and os.path.exists(os.path.join(GOLDEN, "cfg4_src%d_closure1.npz" % s)):
+            golds[s] = _golden(4, s)
     wl = make_config(4)
     K = np.zeros((8, wl.G), dtype=np.int32)                   # 0 = stop by the tolerance
     for s, g in golds.items():
@@ -122,11 +125,12 @@ def test_config4_full_solve_two_sources_against_golden(pkg, capsys):
             assert np.array_equal(pu > 0, lit) and (np.abs(pu[lit] - ref_u[lit]) / ref_u[lit]).max() < 1e-5, (s, grp)
     # the five sources that ran to the tolerance needed about as many sweeps, and converged
     others = [s for s in range(8) if s not in golds]
-    assert (info["residual"][others] < wl.tol).all()
-    assert np.abs(info["iters"][others].astype(int).mean(0) - np.mean([g["iters"] for g in golds.values()], 0)).max() <= 2.0
+    if others:
+        assert (info["residual"][others] < wl.tol).all()
+        assert np.abs(info["iters"][others].astype(int).mean(0) - np.mean([g["iters"] for g in golds.values()], 0)).max() <= 2.0
     with capsys.disabled():
-        print("\n  cfg4 sources 0, 3, 5 full solve (8 sources, 2 chunks of 4): worst rel err %.3e over %d stored cells" % (
-            worst, sum(r[3] for r in report)))
+        print("\n  cfg4 sources %s full solve (8 sources, 2 chunks of 4): worst rel err %.3e over %d stored cells" % (
+            sorted(golds), worst, sum(r[3] for r in report)))
         for s in golds:
             print("   source %d per group max: %s" % (s, " ".join("%.1e" % r[2] for r in report if r[0] == s)))
     assert worst < TOL, [r for r in report if r[2] >= TOL]
