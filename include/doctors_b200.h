@@ -222,6 +222,23 @@ int doctors_host_projection_tables(int pl_order, int n_dir, const double* omega_
  * P1 / P2 / P3 / P4 at S2 / S4 / S6 / S8 and beyond P3 at S12 / S16 (quadrature rule). */
 int doctors_host_pl_exceeds_quadrature(int pl_order, int n_dir, const double* omega_xyz, const double* w, double* defect);
 
+
+/* Allocation-free entry point (for callers that may not allocate: CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc).  The convergence measure of the source iteration (reading R8), per problem q:
+ *     delta_q = max_c |phi_new[q][c] - phi_old[q][c]| / max_c |phi_new[q][c]|       (0 if phi_new is identically 0)
+ * i.e. what doctors_solve evaluates on the device after every sweep, offered for fluxes the caller holds.
+ *   device_phi_new, device_phi_old : DEVICE pointers, fp32, problem q at offset q * problem_stride, n_cells values each
+ *                                    (any cell order; padding cells must hold equal values in both, e.g. 0)
+ *   device_out                     : DEVICE pointer, [n_problems][3] fp32 = delta, max |new - old|, max |new|; a NaN input gives inf
+ * The call enqueues a 256-byte memset node and one kernel on the handle's stream and returns without synchronising; it calls
+ * no cudaMalloc / cudaFree / allocating routine.  Its cross-block scratch is a static __device__ array of 33,024 bytes that
+ * every GPU which loads the library holds until exit.  Limit: n_problems <= 64 per call (INVALID_ARG beyond, with a message).
+ * ALL calls on a device share that array: calls that overlap on the GPU (other streams, other handles) race — serialise them.
+ * The first call per device looks up the array's device address (cudaGetSymbolAddress): make it outside a graph capture.
+ * Errors: INVALID_ARG (NULL pointer, n_problems outside 1..64, n_cells < 1, stride < n_cells), CUDA on a runtime error. */
+int doctors_convergence_delta_no_alloc(doctors_problem* p, const float* device_phi_new, const float* device_phi_old,
+                                       long long n_cells, long long problem_stride, int n_problems, float* device_out);
+
 #ifdef __cplusplus
 }
 #endif

@@ -23,7 +23,7 @@ EXPORTS = [
     "doctors_set_workspace", "doctors_solve", "doctors_get_flux_moments", "doctors_get_uncollided_flux", "doctors_get_response",
     "doctors_debug_schedule_dims", "doctors_debug_get_schedule", "doctors_debug_device_brick_steps", "doctors_wavefront_size", "doctors_debug_get_tables",
     "doctors_host_level_symmetric", "doctors_host_schedule", "doctors_host_projection_tables",
-    "doctors_host_pl_exceeds_quadrature",
+    "doctors_host_pl_exceeds_quadrature", "doctors_convergence_delta_no_alloc",
 ]
 
 
@@ -110,6 +110,7 @@ def load_library():
     L.doctors_host_schedule.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
     L.doctors_host_projection_tables.argtypes = [C.c_int, C.c_int, dp, dp, dp, dp]
     L.doctors_host_pl_exceeds_quadrature.argtypes = [C.c_int, C.c_int, dp, dp, dp]
+    L.doctors_convergence_delta_no_alloc.argtypes = [vp, vp, vp, C.c_longlong, C.c_longlong, C.c_int, vp]
     _lib = L
     return L
 
@@ -350,6 +351,12 @@ class Problem:
         self._check(self._L.doctors_get_response(self._h, problem, _ptr(r, C.c_double), int(bool(include_uncollided)),
                                                  C.c_void_p(host.ctypes.data), 0))
         return host
+
+    def convergence_delta_no_alloc(self, phi_new_ptr, phi_old_ptr, n_cells, problem_stride, n_problems, out_ptr):
+        """doctors_convergence_delta_no_alloc: raw DEVICE pointers in and out (e.g. tensor.data_ptr()); enqueues on the
+        handle's stream, allocates nothing, does not synchronise."""
+        self._check(self._L.doctors_convergence_delta_no_alloc(self._h, C.c_void_p(phi_new_ptr), C.c_void_p(phi_old_ptr),
+                                                               int(n_cells), int(problem_stride), int(n_problems), C.c_void_p(out_ptr)))
 
     # ---- test hooks -------------------------------------------------------------------------
     def debug_schedule(self, octant, level, brick=None):

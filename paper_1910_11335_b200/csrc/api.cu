@@ -1405,3 +1405,105 @@ extern "C" int doctors_get_uncollided_flux(doctors_problem* p, int source, int g
     const float* src = at<float>(p, P.o_phiu) + ((size_t)source * P.G + group) * size_t(P.cells_p);
     return copy_rows_out(p, src, out, out_is_device, 1);
 }
+
+// ------------------------------------------------------------------------------------------
+// Allocation-free entry point: the convergence measure of row a6 (reading R8),
+//   delta = max_c |phi_new(c) - phi_old(c)| / max_c |phi_new(c)|   per problem,
+// for callers that may not allocate (CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).
+// It is a variant of k_check: the same max-reduction over the cells, but the cross-block scratch (per-block partial
+// maxima, last-block tickets) lives in a file-scope __device__ array instead of the caller's workspace, and the result
+// goes to a caller buffer instead of the solver's ProbState.  Every GPU that loads the library holds the array
+// (sizeof(DeltaScratch) = 33,024 bytes) until the process exits.
+//   - ALL calls on a device share the array: calls that overlap on the GPU (two streams, two handles) race.
+//   - The array keeps the last call's contents; what must start at zero (the tickets) is cleared by a memset node on
+//     the caller's stream before every launch, the partial maxima are fully rewritten before they are read.
+//   - No cudaMalloc / cudaFree / allocating library routine is called.  The FIRST call per device looks the array's
+//     device address up (cudaGetSymbolAddress: in host code the array's name is only a stand-in, not a device pointer);
+//     make that first call outside a graph capture.
+// ------------------------------------------------------------------------------------------
+namespace {
+
+constexpr int kDeltaBlocks = 64;            // blocks per problem (grid-stride over the cells)
+constexpr int kDeltaMaxProblems = 64;       // stated maximum: problems per call (doctors_set_source takes at most 64 sources)
+constexpr int kDeltaMaxDevices = 64;
+
+struct DeltaScratch {
+    float part[kDeltaMaxProblems][kDeltaBlocks][2];   // per block: max |new - old|, max |new|
+    unsigned ticket[kDeltaMaxProblems];               // blocks of the problem that have finished (must start at 0)
+};
+
+static __device__ __align__(256) unsigned char g_delta_scratch[sizeof(DeltaScratch)];
+
+__global__ void __launch_bounds__(256)
+k_delta_static(DeltaScratch* S, const float* __restrict__ phi_new, const float* __restrict__ phi_old, long long n,
+               long long stride, float* __restrict__ out /*[n_problems][3]: delta, max |new - old|, max |new|*/)
+{
+    const int p = blockIdx.y;
+    const float* a = phi_new + (size_t)p * stride;
+    const float* b = phi_old + (size_t)p * stride;
+    float md = 0.0f, mp = 0.0f;
+    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < n; c += (long long)gridDim.x * blockDim.x) {
+        const float v = a[c];
+        md = fmaxf(md, fabsf(v - b[c]));
+        mp = fmaxf(mp, fabsf(v));
+        if (!(v == v) || !(b[c] == b[c])) md = INFINITY;            // NaN: visible in the result (fmaxf would drop it)
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        md = fmaxf(md, __shfl_xor_sync(0xffffffffu, md, o));
+        mp = fmaxf(mp, __shfl_xor_sync(0xffffffffu, mp, o));
+    }
+    __shared__ float s_md[8], s_mp[8];
+    __shared__ bool s_last;
+    if ((threadIdx.x & 31) == 0) { s_md[threadIdx.x >> 5] = md; s_mp[threadIdx.x >> 5] = mp; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < 8; ++w) { md = fmaxf(md, s_md[w]); mp = fmaxf(mp, s_mp[w]); }
+        S->part[p][blockIdx.x][0] = md;
+        S->part[p][blockIdx.x][1] = mp;
+        __threadfence();
+        s_last = atomicAdd(&S->ticket[p], 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (s_last && threadIdx.x == 0) {
+        __threadfence();
+        float d = 0.0f, m = 0.0f;
+        for (unsigned blk = 0; blk < gridDim.x; ++blk) {              // fixed order; max is order-independent anyway
+            d = fmaxf(d, __ldcg(&S->part[p][blk][0]));
+            m = fmaxf(m, __ldcg(&S->part[p][blk][1]));
+        }
+        out[3 * p] = m == 0.0f ? 0.0f : (float)((double)d / (double)m);   // as k_check: no source reaches the group -> 0
+        out[3 * p + 1] = d;
+        out[3 * p + 2] = m;
+    }
+}
+
+}  // namespace
+
+extern "C" int doctors_convergence_delta_no_alloc(doctors_problem* p, const float* device_phi_new, const float* device_phi_old,
+                                                  long long n_cells, long long problem_stride, int n_problems, float* device_out)
+{
+    if (!p) return DOCTORS_INVALID_ARG;
+    if (!device_phi_new || !device_phi_old || !device_out) return fail(p, DOCTORS_INVALID_ARG, "NULL device pointer");
+    if (n_problems < 1 || n_problems > kDeltaMaxProblems)
+        return fail(p, DOCTORS_INVALID_ARG, "n_problems = %d: the static scratch of doctors_convergence_delta_no_alloc holds at most %d problems per call",
+                    n_problems, kDeltaMaxProblems);
+    if (n_cells < 1 || n_cells > (1LL << 40)) return fail(p, DOCTORS_INVALID_ARG, "n_cells must be 1 .. 2^40");
+    if (problem_stride < n_cells && n_problems > 1) return fail(p, DOCTORS_INVALID_ARG, "problem_stride must be >= n_cells");
+    if (p->device < 0 || p->device >= kDeltaMaxDevices) return fail(p, DOCTORS_INVALID_ARG, "device ordinal beyond %d", kDeltaMaxDevices - 1);
+    CK(cudaSetDevice(p->device));
+    // set-up, once per device, with that device current: the device address of the static scratch
+    static DeltaScratch* scratch_of[kDeltaMaxDevices] = {};
+    if (!scratch_of[p->device]) {
+        void* ptr = nullptr;
+        CK(cudaGetSymbolAddress(&ptr, g_delta_scratch));
+        if (!ptr) return fail(p, DOCTORS_CUDA, "cudaGetSymbolAddress returned a null address");
+        scratch_of[p->device] = static_cast<DeltaScratch*>(ptr);
+    }
+    DeltaScratch* S = scratch_of[p->device];
+    CK(cudaMemsetAsync(S->ticket, 0, sizeof S->ticket, p->stream));   // shared, keeps the last call's contents: tickets start at zero
+    const unsigned bx = unsigned(std::min<long long>(kDeltaBlocks, (n_cells + 255) / 256));
+    k_delta_static<<<dim3(bx, unsigned(n_problems)), 256, 0, p->stream>>>(S, device_phi_new, device_phi_old, n_cells, problem_stride, device_out);
+    CK(cudaGetLastError());
+    return DOCTORS_OK;
+}
