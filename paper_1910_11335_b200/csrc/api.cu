@@ -1324,7 +1324,7 @@ extern "C" int doctors_debug_device_brick_steps(doctors_problem* p, int bx, int 
     bp.M = 1; bp.W = 1; bp.g = 0; bp.Gs = 1; bp.epoch = 1; bp.task_begin = 0; bp.ntasks = 1; bp.counter_slot = 0;
     bp.NCb = NC; bp.cells_p = NC; bp.Q = S.Q; bp.phi = S.phi; bp.sigt = S.sig; bp.octtab = S.tab;
     bp.tasks = S.task; bp.ctl = S.ctl; bp.flags = S.flags;
-    bp.faceX = S.face; bp.faceY = S.face + size_t(by) * bz; bp.faceZ = bp.faceY + size_t(bx) * bz;
+    bp.faceX = S.face; bp.faceY = S.face + size_t(by) * bz; bp.faceZ = S.face + size_t(by) * bz + size_t(bx) * bz;   // element offsets (fp64 faces: closure 0)
     bp.state = S.st; bp.leak = S.leak;
     bp.dbg_plane = S.planes;
     cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<1, false, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
