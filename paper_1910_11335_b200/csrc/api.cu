@@ -707,19 +707,37 @@ int make_tensor_map(doctors_problem* p, CUtensorMap* tm, void* base, int rank, c
     return DOCTORS_OK;
 }
 
+// the fixed-pitch instantiation (sweep_brick.cuh, PITCH = 640) exists for P3 with the FMA-loop projections
+constexpr int kFixedPitch = 640;
+template <int NM, int MT>
+constexpr bool has_fixed_pitch() { return NM == 16 && MT == 0; }
+
 template <int NM, bool FIX, int MT>
 cudaError_t launch_brick(const SweepLaunch& S, cudaStream_t st)
 {
-    k_sweep_brick<NM, FIX, MT><<<S.grid, 32 * S.bp.W, S.smem, st>>>(S.tmQ, S.tmPhi, S.bp);
+    if constexpr (has_fixed_pitch<NM, MT>()) {
+        if (S.bp.NCb == kFixedPitch) {
+            k_sweep_brick<NM, FIX, MT, kFixedPitch><<<S.grid, 32 * S.bp.W, S.smem, st>>>(S.tmQ, S.tmPhi, S.bp);
+            return cudaGetLastError();
+        }
+    }
+    k_sweep_brick<NM, FIX, MT, 0><<<S.grid, 32 * S.bp.W, S.smem, st>>>(S.tmQ, S.tmPhi, S.bp);
     return cudaGetLastError();
 }
 
 template <int NM, bool FIX, int MT>
-cudaError_t prep_brick(size_t smem, int threads, int* max_ctas)
+cudaError_t prep_brick(int ncb, size_t smem, int threads, int* max_ctas)
 {
-    cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<NM, FIX, MT>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+    if constexpr (has_fixed_pitch<NM, MT>()) {
+        if (ncb == kFixedPitch) {
+            cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<NM, FIX, MT, kFixedPitch>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+            if (e != cudaSuccess) return e;
+            return cudaOccupancyMaxActiveBlocksPerMultiprocessor(max_ctas, k_sweep_brick<NM, FIX, MT, kFixedPitch>, threads, smem);
+        }
+    }
+    cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<NM, FIX, MT, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(max_ctas, k_sweep_brick<NM, FIX, MT>, threads, smem);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(max_ctas, k_sweep_brick<NM, FIX, MT, 0>, threads, smem);
 }
 
 // NM in {1, 4, 9, 16}; MT > 0 only with NM = 16 (projection_mtiles)
@@ -939,7 +957,7 @@ int prepare(doctors_problem* p, const doctors_solve_opts& o, const Plan& P)
         }
         int max_ctas = 0;
         cudaError_t e = cudaSuccess;
-        DISPATCH_NM_FIX(NM, o.closure == 1, P.MT, e = (prep_brick<NM, FIX, MT>(P.smem, 32 * P.W, &max_ctas)));
+        DISPATCH_NM_FIX(NM, o.closure == 1, P.MT, e = (prep_brick<NM, FIX, MT>(P.NCb, P.smem, 32 * P.W, &max_ctas)));
         if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "sweep kernel setup failed: %s (smem %zu)", cudaGetErrorString(e), P.smem);
         if (max_ctas < 1) return fail(p, DOCTORS_CUDA, "sweep kernel does not fit an SM (smem %zu)", P.smem);
         ctas_per_sm = o.ctas_per_sm > 0 ? std::min(o.ctas_per_sm, max_ctas) : max_ctas;
@@ -1327,9 +1345,9 @@ extern "C" int doctors_debug_device_brick_steps(doctors_problem* p, int bx, int 
     bp.faceX = S.face; bp.faceY = S.face + size_t(by) * bz; bp.faceZ = S.face + size_t(by) * bz + size_t(bx) * bz;   // element offsets (fp64 faces: closure 0)
     bp.state = S.st; bp.leak = S.leak;
     bp.dbg_plane = S.planes;
-    cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<1, false, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+    cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<1, false, 0, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
     if (e == cudaSuccess) {
-        k_sweep_brick<1, false, 0, true><<<1, 32, smem, p->stream>>>(SL.tmQ, SL.tmPhi, bp);
+        k_sweep_brick<1, false, 0, 0, true><<<1, 32, smem, p->stream>>>(SL.tmQ, SL.tmPhi, bp);
         e = cudaGetLastError();
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);

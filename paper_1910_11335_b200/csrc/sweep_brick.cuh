@@ -128,7 +128,7 @@ __host__ __device__ inline BrickSmem brick_smem_layout(int NM, int BX, int BY, i
 {
     BrickSmem s;
     size_t NC = size_t(BX) * BY * BZ, o = 0;
-    s.misc = o;  o = align_up(o + 128, 128);   // mbarrier, task slots, reduction scratch
+    s.misc = o;  o = align_up(o + 256, 128);   // mbarriers, reduction scratch, two decoded task slots (TaskSlot) at +128
     // front pad: a wavefront lane that has not reached its x range yet loads from its running address, up to
     // (BY + BZ - 2) steps of BY cells (8 bytes each for sigma_t) BEFORE its row — that must still be this CTA's memory
     o = align_up(o + size_t(8) * BY * (BY + BZ - 2), 128);
@@ -311,7 +311,23 @@ __device__ __noinline__ void project_directions_to_moments_mma(uint32_t tile, ui
     }
 }
 
-template <int NM, bool FIX, int MT, bool DBG = false>
+// A task as the sweeping warps consume it: decoded ONCE by the thread that fetches it (while the previous task runs) instead of
+// by every warp of the CTA (the decode was ~100 instructions per warp and task, 8 % of all instructions executed: profiles/).
+struct __align__(16) TaskSlot {
+    int id;                        // position in the task list (>= ntasks: no more work)
+    unsigned bits;                 // prob | oct << 8 | upx, upy, upz, dnx, dny, dnz << 16.. | stopped << 24
+    int brick;
+    unsigned ext;                  // clipped extents ex | ey << 8 | ez << 16
+    unsigned long long gFx, gFy, gFz;   // this brick's face blocks in the global exchange buffers
+    unsigned long long flag_base;       // done-flags of (prob, oct): [bricks]
+    unsigned long long pad;
+};
+static_assert(sizeof(TaskSlot) == 64, "two slots fit the misc area");
+
+// PITCH > 0: the brick holds exactly PITCH cells (the default 20 x 8 x 4 = 640) and the plane pitch of the tile is a compile-time
+// constant: the 32 plane addresses a thread touches in each projection become immediates off one base register (they were an
+// IMAD each).  PITCH = 0: any brick, pitch from the parameters.  The brick's EXTENTS stay run-time values either way.
+template <int NM, bool FIX, int MT, int PITCH, bool DBG = false>
 __global__ void __launch_bounds__(32 * kMaxSweepWarps, 3)
 k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmPhi, const BrickParams P)
 {
@@ -320,8 +336,9 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
     if (__ldcg(&P.ctl->all_done)) return;                              // every problem of the chunk has stopped (a6): nothing to sweep
     extern __shared__ __align__(128) unsigned char smem[];
     const int BX = P.BX, BY = P.BY, BZ = P.BZ, M = P.M;
-    const int NC = BX * BY * BZ;
-    const int NCP = plane_pitch(NC, MT);                              // plane pitch of the tile (floats)
+    static_assert(PITCH == 0 || MT == 0, "a fixed pitch is instantiated for the dense (FMA-loop) tile only");
+    const int NC = PITCH ? PITCH : BX * BY * BZ;
+    const int NCP = PITCH ? PITCH : plane_pitch(NC, MT);              // plane pitch of the tile (floats)
     using face_t = typename FaceOf<FIX>::type;
     constexpr unsigned kFaceBytes = sizeof(face_t);
     const BrickSmem L = brick_smem_layout(NM, BX, BY, BZ, M, MT, kFaceBytes);
@@ -337,7 +354,6 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
     float* sM = reinterpret_cast<float*>(smem + L.tab + T.t0);      // MT = 0: [M][pitch];  MT >= 1: A fragments (float4 per lane)
     float* sD = reinterpret_cast<float*>(smem + L.tab + T.t2);
     uint64_t* sBar = reinterpret_cast<uint64_t*>(smem + L.misc);
-    int* sTask = reinterpret_cast<int*>(smem + L.misc + 8);
     float* sRed = reinterpret_cast<float*>(smem + L.misc + 64);     // kMaxSweepWarps floats
 
     const int tid = threadIdx.x, nthr = blockDim.x;
@@ -367,46 +383,58 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
     const int tileWarp = nwarps > 1 ? 1 : 0;
     const int pfThread = nwarps > 2 ? 64 : 32 * tileWarp + 8;
     const int pubWarp = nwarps - 1;
-    uint2* sDesc = reinterpret_cast<uint2*>(smem + L.misc + 16);   // [2]
+    TaskSlot* sSlot = reinterpret_cast<TaskSlot*>(smem + L.misc + 128);   // [2]
     unsigned char* sDoneP = smem + L.done;                        // [nprob]: fixed for the whole launch (k_check runs between launches)
     for (int q = tid; q < P.nprob; q += nthr) sDoneP[q] = (unsigned char)(__ldcg(&P.state[q].done) != 0);
     auto fetch_task = [&](int sl) {
         const int id = int(atomicAdd(&P.ctl->counters[P.counter_slot], 1u));
-        uint2 d = make_uint2(0u, 0u);
-        if (id < P.ntasks) d = P.tasks[P.task_begin + id];
-        sDesc[sl] = d; sTask[sl] = id;
+        TaskSlot t;
+        t.id = id; t.bits = 0u; t.brick = 0; t.ext = 0u; t.gFx = t.gFy = t.gFz = t.flag_base = t.pad = 0ull;
+        if (id < P.ntasks) {
+            const uint2 d = P.tasks[P.task_begin + id];
+            const int prob = d.x & 0xff, oct = (d.x >> 8) & 7;
+            const int bi = d.y & 0x3ff, bj = (d.y >> 10) & 0x3ff, bk = (d.y >> 20) & 0x3ff;
+            const int ex = min(BX, P.nx - bi * BX), ey = min(BY, P.ny - bj * BY), ez = min(BZ, P.nz - bk * BZ);   // clipped extents
+            const bool px = !(oct & 1), py_ = !(oct & 2), pz_ = !(oct & 4);
+            const unsigned upx = px ? bi > 0 : bi < P.gbx - 1, upy = py_ ? bj > 0 : bj < P.gby - 1, upz = pz_ ? bk > 0 : bk < P.gbz - 1;
+            const unsigned dnx = px ? bi < P.gbx - 1 : bi > 0, dny = py_ ? bj < P.gby - 1 : bj > 0, dnz = pz_ ? bk < P.gbz - 1 : bk > 0;
+            t.bits = unsigned(prob) | unsigned(oct) << 8 | upx << 16 | upy << 17 | upz << 18 | dnx << 19 | dny << 20 | dnz << 21 |
+                     unsigned(sDoneP[prob]) << 24;
+            t.brick = bi + P.gbx * (bj + P.gby * bk);
+            t.ext = unsigned(ex) | unsigned(ey) << 8 | unsigned(ez) << 16;
+            const size_t po = (size_t)prob * 8 + oct;
+            t.gFx = reinterpret_cast<unsigned long long>(static_cast<face_t*>(P.faceX) + (po * (P.gby * P.gbz) + bj + P.gby * bk) * (size_t)faceXn);
+            t.gFy = reinterpret_cast<unsigned long long>(static_cast<face_t*>(P.faceY) + (po * (P.gbx * P.gbz) + bi + P.gbx * bk) * (size_t)faceYn);
+            t.gFz = reinterpret_cast<unsigned long long>(static_cast<face_t*>(P.faceZ) + (po * (P.gbx * P.gby) + bi + P.gbx * bj) * (size_t)faceZn);
+            t.flag_base = reinterpret_cast<unsigned long long>(P.flags + po * (size_t)nbricks);
+        }
+        sSlot[sl] = t;
     };
+    __syncthreads();                                             // stop flags (read by fetch_task)
     if (tid == 0) fetch_task(0);
-    __syncthreads();                                             // mbarriers, first task, stop flags
+    __syncthreads();                                             // mbarriers, first task
     int slot = 0;
     // ONE block barrier ends a task (after phase 2): behind it nobody reads the tile, the tables, the faces or the task
     // slot of that task any more, so the next task starts without a barrier of its own.
     while (true) {
-        const int t = sTask[slot];
+        const TaskSlot& ts = sSlot[slot];
+        const int t = ts.id;
         if (t >= P.ntasks) break;
-        const uint2 td = sDesc[slot];
-        const int prob_done = sDoneP[td.x & 0xff];
+        const unsigned tb = ts.bits;
         if (tid == pfThread) fetch_task(slot ^ 1);
         slot ^= 1;
-        if (prob_done) { __syncthreads(); continue; }            // this problem has stopped (a6); the barrier orders the task slots
-        const int prob = td.x & 0xff, oct = (td.x >> 8) & 7;
-        const int bi = td.y & 0x3ff, bj = (td.y >> 10) & 0x3ff, bk = (td.y >> 20) & 0x3ff;
-
-        const int x0 = bi * BX, y0 = bj * BY, z0 = bk * BZ;
-        const int ex = min(BX, P.nx - x0), ey = min(BY, P.ny - y0), ez = min(BZ, P.nz - z0);   // clipped extents
+        if (tb >> 24) { __syncthreads(); continue; }             // this problem has stopped (a6); the barrier orders the task slots
+        const int prob = tb & 0xff, oct = (tb >> 8) & 7;
+        const unsigned te = ts.ext;
+        const int ex = te & 0xff, ey = (te >> 8) & 0xff, ez = te >> 16;
         const int sx = (oct & 1) ? -1 : 1, sy = (oct & 2) ? -1 : 1, sz = (oct & 4) ? -1 : 1;
-        const bool upx = sx > 0 ? bi > 0 : bi < P.gbx - 1;
-        const bool upy = sy > 0 ? bj > 0 : bj < P.gby - 1;
-        const bool upz = sz > 0 ? bk > 0 : bk < P.gbz - 1;
-        const bool dnx = sx > 0 ? bi < P.gbx - 1 : bi > 0;      // a downwind brick exists
-        const bool dny = sy > 0 ? bj < P.gby - 1 : bj > 0;
-        const bool dnz = sz > 0 ? bk < P.gbz - 1 : bk > 0;
-        const int brick = bi + P.gbx * (bj + P.gby * bk);
-        unsigned* flag_base = P.flags + (size_t)(prob * 8 + oct) * nbricks;
-        const size_t po = (size_t)prob * 8 + oct;
-        face_t* gFx = static_cast<face_t*>(P.faceX) + (po * (P.gby * P.gbz) + bj + P.gby * bk) * (size_t)faceXn;
-        face_t* gFy = static_cast<face_t*>(P.faceY) + (po * (P.gbx * P.gbz) + bi + P.gbx * bk) * (size_t)faceYn;
-        face_t* gFz = static_cast<face_t*>(P.faceZ) + (po * (P.gbx * P.gby) + bi + P.gbx * bj) * (size_t)faceZn;
+        const bool upx = (tb >> 16) & 1, upy = (tb >> 17) & 1, upz = (tb >> 18) & 1;
+        const bool dnx = (tb >> 19) & 1, dny = (tb >> 20) & 1, dnz = (tb >> 21) & 1;      // a downwind brick exists
+        const int brick = ts.brick;
+        unsigned* flag_base = reinterpret_cast<unsigned*>(ts.flag_base);
+        face_t* gFx = reinterpret_cast<face_t*>(ts.gFx);
+        face_t* gFy = reinterpret_cast<face_t*>(ts.gFy);
+        face_t* gFz = reinterpret_cast<face_t*>(ts.gFz);
 
         // tile, sigma_t and (when the octant changes) the octant's table blob: bulk async copies, one mbarrier.
         // Directions of an octant are contiguous (n = oct*M + m); nobody reads the old tables any more (loop-top barrier).
