@@ -707,7 +707,8 @@ int make_tensor_map(doctors_problem* p, CUtensorMap* tm, void* base, int rank, c
     return DOCTORS_OK;
 }
 
-// the fixed-pitch instantiation (sweep_brick.cuh, PITCH = 640) exists for P3 with the FMA-loop projections
+// the fixed-pitch instantiation (sweep_brick.cuh, PITCH = 640: 640-cell bricks, 10 directions per octant) exists for P3 with the
+// FMA-loop projections: the shapes of configs 1, 2 and 4
 constexpr int kFixedPitch = 640;
 template <int NM, int MT>
 constexpr bool has_fixed_pitch() { return NM == 16 && MT == 0; }
@@ -716,7 +717,7 @@ template <int NM, bool FIX, int MT>
 cudaError_t launch_brick(const SweepLaunch& S, cudaStream_t st)
 {
     if constexpr (has_fixed_pitch<NM, MT>()) {
-        if (S.bp.NCb == kFixedPitch) {
+        if (S.bp.NCb == kFixedPitch && S.bp.M == 10) {
             k_sweep_brick<NM, FIX, MT, kFixedPitch><<<S.grid, 32 * S.bp.W, S.smem, st>>>(S.tmQ, S.tmPhi, S.bp);
             return cudaGetLastError();
         }
@@ -726,10 +727,10 @@ cudaError_t launch_brick(const SweepLaunch& S, cudaStream_t st)
 }
 
 template <int NM, bool FIX, int MT>
-cudaError_t prep_brick(int ncb, size_t smem, int threads, int* max_ctas)
+cudaError_t prep_brick(int ncb, int m_oct, size_t smem, int threads, int* max_ctas)
 {
     if constexpr (has_fixed_pitch<NM, MT>()) {
-        if (ncb == kFixedPitch) {
+        if (ncb == kFixedPitch && m_oct == 10) {
             cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<NM, FIX, MT, kFixedPitch>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
             if (e != cudaSuccess) return e;
             return cudaOccupancyMaxActiveBlocksPerMultiprocessor(max_ctas, k_sweep_brick<NM, FIX, MT, kFixedPitch>, threads, smem);
@@ -957,7 +958,7 @@ int prepare(doctors_problem* p, const doctors_solve_opts& o, const Plan& P)
         }
         int max_ctas = 0;
         cudaError_t e = cudaSuccess;
-        DISPATCH_NM_FIX(NM, o.closure == 1, P.MT, e = (prep_brick<NM, FIX, MT>(P.NCb, P.smem, 32 * P.W, &max_ctas)));
+        DISPATCH_NM_FIX(NM, o.closure == 1, P.MT, e = (prep_brick<NM, FIX, MT>(P.NCb, P.M, P.smem, 32 * P.W, &max_ctas)));
         if (e != cudaSuccess) return fail(p, DOCTORS_CUDA, "sweep kernel setup failed: %s (smem %zu)", cudaGetErrorString(e), P.smem);
         if (max_ctas < 1) return fail(p, DOCTORS_CUDA, "sweep kernel does not fit an SM (smem %zu)", P.smem);
         ctas_per_sm = o.ctas_per_sm > 0 ? std::min(o.ctas_per_sm, max_ctas) : max_ctas;

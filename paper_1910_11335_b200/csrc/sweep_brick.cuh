@@ -326,7 +326,9 @@ static_assert(sizeof(TaskSlot) == 64, "two slots fit the misc area");
 
 // PITCH > 0: the brick holds exactly PITCH cells (the default 20 x 8 x 4 = 640) and the plane pitch of the tile is a compile-time
 // constant: the 32 plane addresses a thread touches in each projection become immediates off one base register (they were an
-// IMAD each).  PITCH = 0: any brick, pitch from the parameters.  The brick's EXTENTS stay run-time values either way.
+// IMAD each), and the octant has 10 directions (S8: the projection loops have a constant trip count).  PITCH = 0: any brick and
+// quadrature, from the parameters.  The brick's EXTENTS and the thread count stay run-time values either way (as constants they
+// cost more in spills at the 64-register cap than they save: measured 8.59 against 8.31 ms).
 template <int NM, bool FIX, int MT, int PITCH, bool DBG = false>
 __global__ void __launch_bounds__(32 * kMaxSweepWarps, 3)
 k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmPhi, const BrickParams P)
@@ -335,7 +337,7 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
     static_assert(NM <= 16, "one tile-warp lane per moment plane, lanes 16 / 17 for sigma_t and the tables");
     if (__ldcg(&P.ctl->all_done)) return;                              // every problem of the chunk has stopped (a6): nothing to sweep
     extern __shared__ __align__(128) unsigned char smem[];
-    const int BX = P.BX, BY = P.BY, BZ = P.BZ, M = P.M;
+    const int BX = P.BX, BY = P.BY, BZ = P.BZ, M = PITCH ? 10 : P.M;   // fixed pitch: S8, 10 directions per octant
     static_assert(PITCH == 0 || MT == 0, "a fixed pitch is instantiated for the dense (FMA-loop) tile only");
     const int NC = PITCH ? PITCH : BX * BY * BZ;
     const int NCP = PITCH ? PITCH : plane_pitch(NC, MT);              // plane pitch of the tile (floats)
