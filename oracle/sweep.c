@@ -237,6 +237,12 @@ void orc_sweep(int nx, int ny, int nz, double dx, double dy, double dz,
     free(psi_buf); free(qn_buf); free(leak_n); free(nfix_n);
 }
 
+static int cmp_double(const void *a, const void *b)
+{
+    double x = *(const double *)a, y = *(const double *)b;
+    return (x > y) - (x < y);
+}
+
 /* ---- PAPER.md:44-49 Eq. (4): uncollided fluence by ray tracing (reading R11, R12) ----
  * For every cell centre r_c:  d = r_c - r_s, R = |d|, u = d/R.
  *   kind 2 (cone): u . axis >= cos_half, else phi_u = 0.
@@ -245,10 +251,11 @@ void orc_sweep(int nx, int ny, int nz, double dx, double dy, double dz,
  *   perpendicular to a) and t = n x a, the direction u has the polar angle beta = asin(u . n) out of the plane
  *   and the azimuth alpha = atan2(u . t, u . a) in it; lit iff |beta| <= half2 and |alpha| <= half, i.e.
  *   |u . n| <= sin_half2 and u . a >= cos_half * sqrt((u . a)^2 + (u . t)^2).  Hard edges, 4 pi kept (R12).
- *   The segment [0,R] is clipped to the mesh box (outside is vacuum) and walked voxel by
- *   voxel (parametric traversal: per axis the next boundary crossing tMax and the step
- *   tDelta; always step the axis with the smallest tMax).  Per material m the areal
- *   density A_m = sum rho * length is accumulated (independent of the group), then
+ *   The segment [0,R] is clipped to the mesh box (outside is vacuum), cut at every grid plane it crosses (crossing
+ *   parameters computed plane by plane, then sorted) and every piece is assigned to the voxel its midpoint lies in.  The
+ *   library's kernel walks the same path incrementally (running tMax / tDelta per axis): the two agree to rounding, and
+ *   an error in either traversal shows up in the comparison.  Per material m the areal density A_m = sum rho * length
+ *   is accumulated (independent of the group), then
  *     tau_g = sum_m sigt_hat[m][g] A_m,   phi_u^g = S_g exp(-tau_g) / (4 pi R^2).
  * mesh centred on the origin.  phi_u [G][cells]; areal NULL or [n_mat][cells]. */
 void orc_raytrace(int nx, int ny, int nz, double dx, double dy, double dz,
@@ -288,36 +295,54 @@ void orc_raytrace(int nx, int ny, int nz, double dx, double dy, double dz,
             if (ua < cos_half * sqrt(ua * ua + ut * ut)) lit = 0;
         }
         if (lit) {
-            /* clip [0,R] to the box: entry parameter */
-            double t0 = 0.0;
+            /* The radiological path written out as its definition (reading R11): the part of the segment [0, R] inside the
+             * mesh box is cut at EVERY grid plane it crosses, x, y and z planes alike; the crossing parameters are computed
+             * one by one from the plane positions and sorted; each piece between two consecutive crossings lies in one voxel,
+             * found from the piece's midpoint, and adds rho * length to that voxel's material.  (No incremental stepping,
+             * no running tMax / tDelta, no tie-breaking: a ray through a voxel edge gives a zero-length piece.) */
+            double t0 = 0.0, t1 = R;                                /* in-box interval by slab clipping */
             for (int a = 0; a < 3; ++a) {
-                if (u[a] > 0.0) { double t = (lo[a] - spos[a]) / u[a]; if (t > t0) t0 = t; }
-                else if (u[a] < 0.0) { double t = (lo[a] + nn[a] * del[a] - spos[a]) / u[a]; if (t > t0) t0 = t; }
+                double hi_a = lo[a] + nn[a] * del[a];
+                if (u[a] != 0.0) {
+                    double ta = (lo[a] - spos[a]) / u[a], tb = (hi_a - spos[a]) / u[a];
+                    double tnear = ta < tb ? ta : tb, tfar = ta < tb ? tb : ta;
+                    if (tnear > t0) t0 = tnear;
+                    if (tfar < t1) t1 = tfar;
+                } else if (spos[a] < lo[a] || spos[a] > hi_a) t1 = -1.0;   /* parallel to the slab and outside it */
             }
-            int idx[3], step[3];
-            double tmax[3], tdel[3];
-            for (int a = 0; a < 3; ++a) {
-                double p = spos[a] + t0 * u[a];
-                int ii = (int)floor((p - lo[a]) / del[a]);
-                if (ii < 0) ii = 0;
-                if (ii > nn[a] - 1) ii = nn[a] - 1;
-                idx[a] = ii;
-                if (u[a] > 0.0) { step[a] = 1; tmax[a] = (lo[a] + (ii + 1) * del[a] - spos[a]) / u[a]; tdel[a] = del[a] / u[a]; }
-                else if (u[a] < 0.0) { step[a] = -1; tmax[a] = (lo[a] + ii * del[a] - spos[a]) / u[a]; tdel[a] = -del[a] / u[a]; }
-                else { step[a] = 0; tmax[a] = INFINITY; tdel[a] = INFINITY; }
-            }
-            double t = t0;
-            for (int it = 0; it < nx + ny + nz + 4 && t < R; ++it) {
-                int a = 0;
-                if (tmax[1] < tmax[a]) a = 1;
-                if (tmax[2] < tmax[a]) a = 2;
-                double tn = tmax[a] < R ? tmax[a] : R;
-                size_t v = (size_t)idx[0] + (size_t)nx * (idx[1] + (size_t)ny * idx[2]);
-                if (tn > t) A[mat[v]] += rho[v] * (tn - t);
-                t = tn;
-                idx[a] += step[a];
-                tmax[a] += tdel[a];
-                if (idx[a] < 0 || idx[a] >= nn[a]) break;
+            if (t1 > t0) {
+                double *tc = (double *)malloc(sizeof(double) * (size_t)(nx + ny + nz + 8));
+                int n = 0;
+                tc[n++] = t0;
+                for (int a = 0; a < 3; ++a) {
+                    if (u[a] == 0.0) continue;
+                    /* planes between the two end points of the in-box piece (one spare on each side) */
+                    double pa = (spos[a] + t0 * u[a] - lo[a]) / del[a], pb = (spos[a] + t1 * u[a] - lo[a]) / del[a];
+                    int p_lo = (int)floor(pa < pb ? pa : pb) - 1, p_hi = (int)ceil(pa < pb ? pb : pa) + 1;
+                    if (p_lo < 0) p_lo = 0;
+                    if (p_hi > nn[a]) p_hi = nn[a];
+                    for (int pl = p_lo; pl <= p_hi; ++pl) {
+                        double t = (lo[a] + pl * del[a] - spos[a]) / u[a];
+                        if (t > t0 && t < t1) tc[n++] = t;
+                    }
+                }
+                tc[n++] = t1;
+                qsort(tc, (size_t)n, sizeof(double), cmp_double);
+                for (int i = 0; i + 1 < n; ++i) {
+                    double len = tc[i + 1] - tc[i];
+                    if (!(len > 0.0)) continue;
+                    double tm = 0.5 * (tc[i] + tc[i + 1]);
+                    int vi[3];
+                    for (int a = 0; a < 3; ++a) {
+                        int ii = (int)floor((spos[a] + tm * u[a] - lo[a]) / del[a]);
+                        if (ii < 0) ii = 0;
+                        if (ii > nn[a] - 1) ii = nn[a] - 1;
+                        vi[a] = ii;
+                    }
+                    size_t v = (size_t)vi[0] + (size_t)nx * (vi[1] + (size_t)ny * vi[2]);
+                    A[mat[v]] += rho[v] * len;
+                }
+                free(tc);
             }
         }
         for (int m = 0; m < n_mat && areal; ++m) areal[(size_t)m * cells + c] = A[m];
