@@ -270,3 +270,22 @@ def test_raytrace_sphere_chords_config1(orc):
     assert central.any() and np.abs(water[central] - 12.0).max() < 0.55
     miss = (b2 > 49.0)
     assert (water[miss] == 0.0).all()
+
+
+def test_source_iteration_contracts_at_most_at_the_scattering_ratio(orc):
+    """SURVEY 8(c) pin table, "Iteration": delta_k decreases geometrically at a rate <= the in-group scattering ratio c =
+    sigma_s,gg / sigma_t (source iteration's error contracts by at most c per sweep in any medium; leakage only helps), and the
+    sweep count does not depend on how the sources are chunked (the oracle has no chunks: one problem at a time)."""
+    wl = make_config(1)
+    wl.G = 2
+    wl.sigma_t = wl.sigma_t[:, 8:10].copy(); wl.sigma_s = wl.sigma_s[:, :, 8:10, 8:10].copy()
+    wl.sources[0].spectrum = np.array([0.5, 0.5])
+    wl.tol = 1e-9
+    res = orc.solve(wl, closure=0, keep_history=True)
+    for g in range(2):
+        c = (wl.sigma_s[:, 0, g, g] / wl.sigma_t[:, g]).max()       # the same ratio in every material of the synthetic tables
+        h = res["history"][0][g]
+        assert len(h) >= 8 and h[-1] < wl.tol
+        ratios = [h[k + 1] / h[k] for k in range(2, len(h) - 1)]
+        assert max(ratios) <= c + 1e-3, (g, c, max(ratios))
+        assert min(ratios) > 0.02                                     # geometric, not erratic
