@@ -577,10 +577,9 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         const int li0 = (sx > 0 ? 0 : ex - 1) - sx * (jp + kp);   // li at step 0 (i' = -(j'+k')), advanced by sx per step
         const uint32_t row = uint32_t(lj + BY * (li0 + BX * lk_));    // local index: y fastest, then x, then z (device_common.cuh)
         const bool first_y = jp == 0, first_z = kp == 0;
-        // Idle lanes (before / after their x range) load from wherever their running address points — always
-        // inside this CTA's shared memory, which starts with a 128-byte pad and ends with the tables — and
-        // compute on that garbage; only stores and the x-face register are predicated.  Clipped lanes
-        // (beyond ey / ez) stay parked on the tile's first cell.
+        // Idle lanes (before / after their x range) keep advancing their running addresses but touch nothing (masked below); the
+        // pads in front of and behind the tile keep even those addresses inside this CTA's shared memory (the debug
+        // instantiation checks that).  Clipped lanes (beyond ey / ez) stay parked on the tile's first cell.
         int d4 = lane_ok ? 4 * sx * BY : 0, d8 = 2 * d4, d8f = lane_ok ? int(kFaceBytes) * sx : 0;   // one cell along x: tile (fp32), sigma_t (fp64), face rows
         int shy = BY, ly = last_y ? 1 : 0, lz = last_z ? 1 : 0;
         // loop invariants pinned in registers: otherwise the compiler re-derives them every step (constant-bank reads,
@@ -601,16 +600,22 @@ k_sweep_brick(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
                 double b = __shfl_up_sync(0xffffffffu, oy, 1);
                 double cc = __shfl_up_sync(0xffffffffu, oz, shy);
                 const bool act = (unsigned)ip < (unsigned)ex;    // this lane's cell lies on the current sub-sweep plane
-                const float q = lds_f32(pq);
-                const double sg = lds_f64(ps);
-                if (first_y) b = load_face<face_t>(py);
-                if (first_z) cc = load_face<face_t>(pz);
-                double ox;
-                const float psi = dd_cell<FIX>(act, q, sg, cx, cy, cz, cs, ax, b, cc, ox, oy, oz);
-                sts_f32_if(act, pq, psi);
-                store_face_if<face_t>(act && ly, py, oy);
-                store_face_if<face_t>(act && lz, pz, oz);
-                if (act) ax = ox;
+                // Lanes outside their x range are masked off (a divergent branch, not predicated garbage arithmetic).  At equal
+                // clock that costs 1 % (8.36 against 8.27 ms per slice launch), but the whole solve runs under the 1000 W cap and a
+                // third of the lane-steps are idle: masked, the SM clock settles at 1927 instead of 1878 MHz and the solve is 1.2 %
+                // faster (profiles/r02_sweep_ncu.md).  The shuffles above stay outside: every lane takes part in them.
+                if (act) {
+                    const float q = lds_f32(pq);
+                    const double sg = lds_f64(ps);
+                    if (first_y) b = load_face<face_t>(py);
+                    if (first_z) cc = load_face<face_t>(pz);
+                    double ox;
+                    const float psi = dd_cell<FIX>(true, q, sg, cx, cy, cz, cs, ax, b, cc, ox, oy, oz);
+                    sts_f32(pq, psi);
+                    store_face_if<face_t>(ly, py, oy);
+                    store_face_if<face_t>(lz, pz, oz);
+                    ax = ox;
+                }
                 if (DBG) {
                     // debug instantiation (doctors_debug_device_brick_steps): the step at which each cell is visited, and a
                     // bounds check of EVERY shared-memory address of the step, idle lanes included (they load from their
