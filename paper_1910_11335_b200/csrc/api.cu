@@ -709,7 +709,9 @@ int make_tensor_map(doctors_problem* p, CUtensorMap* tm, void* base, int rank, c
 
 // the fixed-pitch instantiation (sweep_brick.cuh, PITCH = 640: 640-cell bricks, 10 directions per octant) exists for P3 with the
 // FMA-loop projections: the shapes of configs 1, 2 and 4
-constexpr int kFixedPitch = 640;
+constexpr int kFixedPitch = 640;        // 20 x 8 x 4 cells (the default brick)
+constexpr int kFixedPitchLong = 768;    // 24 x 8 x 4 cells (opts.brick): fits three CTAs per SM with fp32 exchange faces; whole config-4 solve
+                                        // 15.12 / 15.13 s per step against 15.15 / 15.17 s with the default brick (A/B): not worth a new default
 template <int NM, int MT>
 constexpr bool has_fixed_pitch() { return NM == 16 && MT == 0; }
 
@@ -721,24 +723,31 @@ cudaError_t launch_brick(const SweepLaunch& S, cudaStream_t st)
             k_sweep_brick<NM, FIX, MT, kFixedPitch><<<S.grid, 32 * S.bp.W, S.smem, st>>>(S.tmQ, S.tmPhi, S.bp);
             return cudaGetLastError();
         }
+        if (S.bp.NCb == kFixedPitchLong && S.bp.M == 10) {
+            k_sweep_brick<NM, FIX, MT, kFixedPitchLong><<<S.grid, 32 * S.bp.W, S.smem, st>>>(S.tmQ, S.tmPhi, S.bp);
+            return cudaGetLastError();
+        }
     }
     k_sweep_brick<NM, FIX, MT, 0><<<S.grid, 32 * S.bp.W, S.smem, st>>>(S.tmQ, S.tmPhi, S.bp);
     return cudaGetLastError();
+}
+
+template <int NM, bool FIX, int MT, int PITCH>
+cudaError_t prep_one(size_t smem, int threads, int* max_ctas)
+{
+    cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<NM, FIX, MT, PITCH>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+    if (e != cudaSuccess) return e;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(max_ctas, k_sweep_brick<NM, FIX, MT, PITCH>, threads, smem);
 }
 
 template <int NM, bool FIX, int MT>
 cudaError_t prep_brick(int ncb, int m_oct, size_t smem, int threads, int* max_ctas)
 {
     if constexpr (has_fixed_pitch<NM, MT>()) {
-        if (ncb == kFixedPitch && m_oct == 10) {
-            cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<NM, FIX, MT, kFixedPitch>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
-            if (e != cudaSuccess) return e;
-            return cudaOccupancyMaxActiveBlocksPerMultiprocessor(max_ctas, k_sweep_brick<NM, FIX, MT, kFixedPitch>, threads, smem);
-        }
+        if (ncb == kFixedPitch && m_oct == 10) return prep_one<NM, FIX, MT, kFixedPitch>(smem, threads, max_ctas);
+        if (ncb == kFixedPitchLong && m_oct == 10) return prep_one<NM, FIX, MT, kFixedPitchLong>(smem, threads, max_ctas);
     }
-    cudaError_t e = cudaFuncSetAttribute(k_sweep_brick<NM, FIX, MT, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
-    if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(max_ctas, k_sweep_brick<NM, FIX, MT, 0>, threads, smem);
+    return prep_one<NM, FIX, MT, 0>(smem, threads, max_ctas);
 }
 
 // NM in {1, 4, 9, 16}; MT > 0 only with NM = 16 (projection_mtiles)
