@@ -96,11 +96,11 @@ def test_config3_full_solve_against_golden(pkg, capsys):
     p2.close()
 
 
-def test_config4_full_solve_two_sources_against_golden(pkg, capsys):
+def test_config4_full_solve_against_goldens(pkg, capsys):
     """Config 4 (256x256x128 GRF phantom, 47 groups, P3, S8) as bench.py runs it: 8 cone-beam sources batched in 2 chunks of
-    4.  Sources 0 (axis-aligned beam), 3 (135 degrees; both in the first chunk) and 5 (225 degrees, second chunk) replay the
-    oracle's sweep counts through all 47 groups and are compared on every stored cell; the other five run the device-side
-    convergence test in the same solve."""
+    4.  Every source whose golden is committed (0, 3, 5 with all moments; the others lean: scalar flux) replays the oracle's sweep
+    counts through all 47 groups and is compared on every stored cell; sources without a golden run the device-side convergence
+    test in the same solve."""
     golds = {s: _golden(4, s) for s in (0, 3, 5)}              # required: tests/golden/make_goldens.py writes them
     for s in range(8):                                         # the other sources where their (lean) golden is committed
         if s not in golds and os.path.exists(os.path.join(GOLDEN, "cfg4_src%d_closure1.npz" % s)):
